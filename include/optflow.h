@@ -1,0 +1,141 @@
+/*
+ * optflow.h -- C-ABI of liboptflow.so: the dense optical-flow solve of arxiv/paper_1306_2461
+ * (Gautier & Aider, "Real-time planar flow velocity measurements using an optical flow algorithm
+ * implemented on GPU"), written from scratch as CUDA kernels for NVIDIA B200 (sm_100a).
+ *
+ * The method (sec. 2.4): a local, iterative, gradient-based, windowed sum-of-squared-
+ * differences registration of the Lucas-Kanade family, one vector per pixel, solved by Gauss-Newton
+ * iterations coarse-to-fine over an image pyramid from a zero initial guess.  The step list is
+ * BASELINE.json:5; every point the paper leaves open follows the readings D1..D23 in DESIGN.md.
+ *
+ * Conventions
+ *   - images: H rows x W columns, row-major, dense (pitch == width); pixel (x,y) = (column,row).
+ *   - flow (u,v) in pixels per frame pair with  I2(x+u, y+v) ~= I1(x,y)  (D1).
+ *   - "device pointer" = memory of the CUDA device that was current at of_create; "host pointer"
+ *     = ordinary host memory.  Streams are cudaStream_t passed as void* (NULL = default stream).
+ *   - every int-returning call returns OF_OK (0) or a negative of_status; of_last_error() gives the
+ *     text of the calling thread's last failure.  No C++ exception crosses this boundary.
+ *   - a handle is not thread-safe; distinct handles are independent.  There is no CPU fallback:
+ *     without a usable CUDA device of_create fails.
+ *   - results are bit-reproducible for the same inputs (no atomics in any sum).
+ */
+#ifndef OPTFLOW_H_
+#define OPTFLOW_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct of_context *of_handle;
+
+enum of_window { OF_WINDOW_BOX = 0, OF_WINDOW_GAUSSIAN = 1 };
+enum of_status { OF_OK = 0, OF_ERR_INVALID_ARG = -1, OF_ERR_ALLOC = -2, OF_ERR_CUDA = -3, OF_ERR_STATE = -4 };
+enum of_dtype { OF_DTYPE_F32 = 0, OF_DTYPE_U8 = 1, OF_DTYPE_U16 = 2 };
+enum of_stream_mode { OF_STREAM_CONSECUTIVE = 0, OF_STREAM_PAIRS = 1 };
+
+#define OF_MAX_LEVELS 12
+#define OF_MAX_WINDOW_RADIUS 16
+
+/* ---------------------------------------------------------------------------------------------
+ * The three calls named by the north_star (BASELINE.json:5).
+ * ------------------------------------------------------------------------------------------- */
+
+/* Create a solver for width x height images ("two inputs to the algorithm, besides image size":
+ * n_lev and n_iter; interrogation-window radius).
+ *   levels        >= 1, number of pyramid images INCLUDING the base (D3; eq. 1); level
+ *                 l+1 has size ((W_l+1)/2, (H_l+1)/2).
+ *   window_radius R in [1, OF_MAX_WINDOW_RADIUS]: box of (2R+1)^2 equal weights, or for
+ *                 OF_WINDOW_GAUSSIAN a separable Gaussian truncated at R with sigma = R/3 (D11).
+ *   iterations    >= 1 Gauss-Newton iterations per level (D16: no convergence test).
+ * The coarsest level must be at least (2R+1) x (2R+1).  Allocates all scratch on the current CUDA
+ * device (about 12 fp32 planes of the base size); launches no kernel.  Returns NULL on failure. */
+of_handle of_create(int width, int height, int levels, int window_radius, int iterations, int window_type);
+
+/* Solve one pair.  I1, I2: device pointers, fp32, dense H x W, read-only.  u, v: device pointers,
+ * fp32, dense H x W, write-only (the initial guess is always zero).  Everything is
+ * enqueued on `stream`; the call never synchronises or allocates.  Steps enqueued (DESIGN.md
+ * "Kernels"): pyramid build of both images, zero field at the coarsest level, then per level
+ * coarse-to-fine: x2 flow upsampling, and `iterations` x { warp + gradients + five products +
+ * horizontal window sum ; vertical window sum + damped 2x2 solve + in-place (u,v) update }. */
+int of_compute(of_handle h, const float *I1, const float *I2, float *u, float *v, void *stream);
+
+/* Destroy; waits for the handle's own streams.  NULL is a no-op. */
+void of_destroy(of_handle h);
+
+/* ---------------------------------------------------------------------------------------------
+ * Integer camera frames (8-bit camera; BASELINE.json:8-11).  Same as of_compute but
+ * I1, I2 are device pointers to dense uint8 / uint16 frames, converted exactly (no scaling, D17)
+ * on the device.
+ * ------------------------------------------------------------------------------------------- */
+int of_compute_u8(of_handle h, const uint8_t *I1, const uint8_t *I2, float *u, float *v, void *stream);
+int of_compute_u16(of_handle h, const uint16_t *I1, const uint16_t *I2, float *u, float *v, void *stream);
+
+/* Text of the calling thread's last error ("" if none).  Never NULL. */
+const char *of_last_error(void);
+
+/* Conditioning of the 2x2 solve (D14, D15): relative Levenberg damping lam = eps_rel*tr(G)/2
+ * (default 1e-3) and per-iteration increment clamp in pixels (default 3, cf. eq. 1).
+ * eps_rel >= 0, max_step_px > 0. */
+int of_set_conditioning(of_handle h, float eps_rel, float max_step_px);
+
+/* Replay the per-pair launch sequence as a CUDA graph (default on).  The graph is re-captured when
+ * the caller's pointers change. */
+int of_set_graph(of_handle h, int enable);
+
+/* Validity bytes (1 = tr(G) > 0, D14) of the last iteration at level 0 of the last solve: copies
+ * H x W bytes into the device buffer mask_dev, on `stream`. */
+int of_get_validity(of_handle h, uint8_t *mask_dev, void *stream);
+
+/* Size of pyramid level `level`. */
+int of_level_size(of_handle h, int level, int *width, int *height);
+
+/* Number of kernel launches (graph kernel nodes included) enqueued by the last of_compute* call. */
+int of_last_launch_count(of_handle h);
+
+/* Test / profiling hooks.  State is that left by the last of_compute* on this handle.
+ * of_get_debug_plane copies one dense fp32 plane of level `level` into out_dev:
+ *   which 0,1: pyramid image of I1 / I2;  2,3: final u / v of that level (level 0: the field before
+ *   its last iteration);  4..8: the five horizontally summed product planes left by the last
+ *   products kernel (valid only for the level it ran on);  9: det = a*c - b^2 (level 0 only). */
+int of_get_debug_plane(of_handle h, int level, int which, float *out_dev, void *stream);
+/* Run ONE kernel of the iteration on the handle's internal state of `level`:
+ *   which 0: warp + gradients + products + horizontal sum (K2);  1: vertical sum + solve + update (K3,
+ *   in place on the internal field). */
+int of_run_step(of_handle h, int level, int which, void *stream);
+
+/* Stand-alone single steps (rows a2, a10 of the scope table), dense device buffers. */
+int of_pyramid_down(const float *src, int width, int height, float *dst, void *stream);
+int of_upsample_flow(const float *uc, const float *vc, int wc, int hc, float *u, float *v, int width,
+                     int height, void *stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Frame pipeline (Fig. 4 schemes; "(5)" in BASELINE.json:5): pinned host slots,
+ * cudaMemcpyAsync on a side stream, events; uploading frame k+1 overlaps solving pair k, and the
+ * download of field k overlaps solving pair k+1.
+ *   OF_STREAM_CONSECUTIVE: each submitted frame is converted and pyramided once and used as I2 of
+ *       pair (k-1,k) and I1 of pair (k,k+1) (scheme 1: "each field computation requires only one
+ *       image to be processed"); frame 0 yields no field.
+ *   OF_STREAM_PAIRS: each submit carries two frames (I1 then I2, contiguous) = one independent pair.
+ * ------------------------------------------------------------------------------------------- */
+/* dtype: of_dtype of the frames.  result_on_host != 0: fields are copied to pinned host buffers and
+ * of_stream_result returns HOST pointers; else it returns device pointers. */
+int of_stream_open(of_handle h, int dtype, int mode, int result_on_host);
+/* Pinned host buffer for the next submit (W*H elements, x2 in PAIRS mode); the caller fills it.
+ * Blocks until that slot's previous upload has completed.  NULL on error. */
+void *of_stream_acquire(of_handle h);
+/* Enqueue upload (+ solve + download) of the slot last acquired.  Returns OF_ERR_STATE if more than
+ * two produced fields have not been collected with of_stream_result. */
+int of_stream_submit(of_handle h);
+/* Wait for the oldest uncollected field.  *u, *v point to H x W fp32 (host or device per
+ * of_stream_open), valid until the second-next of_stream_result call.  *pair_index (optional)
+ * receives its 0-based index.  OF_ERR_STATE if nothing is pending. */
+int of_stream_result(of_handle h, const float **u, const float **v, int *pair_index);
+/* Drain and release the pipeline's buffers. */
+int of_stream_close(of_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OPTFLOW_H_ */

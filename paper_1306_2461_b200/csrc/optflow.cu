@@ -1,0 +1,626 @@
+// optflow.cu -- host orchestration and C-ABI (include/optflow.h) of the dense optical-flow solve.
+//
+// Level loop / iteration loop / stream + event wiring / CUDA-graph replay; all arithmetic of the
+// method runs in the kernels of of_kernels.cuh.  No CPU fallback anywhere: every path that cannot
+// reach the GPU returns an error.
+#include "../../include/optflow.h"
+#include "of_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+static_assert(OFK_MAX_R == OF_MAX_WINDOW_RADIUS, "radius limits out of sync");
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char *fmt, ...) __attribute__((format(printf, 2, 3)));
+int fail(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define CU_TRY(expr)                                                                              \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(OF_ERR_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+struct Level { int W, H, pitch; };
+
+// One enqueue of the whole path.  Also the key of the graph cache.
+struct Job {
+    int dtype;                 // of_dtype of rawA/rawB
+    const void *rawA, *rawB;   // frames to convert into pyramid slots cvtA / cvtB (rawB may be NULL)
+    int cvtA, cvtB;            // pyramid slots to (re)build, -1 = none
+    int s1, s2;                // pyramid slots used as I1 / I2
+    float *u_out, *v_out;      // level-0 result, dense
+    bool operator==(const Job &o) const { return memcmp(this, &o, sizeof(Job)) == 0; }
+};
+
+struct GraphEntry { Job job; cudaGraphExec_t exec; unsigned long long stamp; int launches; };
+
+constexpr int N_PYR = 2;       // pyramid slots
+constexpr int N_PIN = 2;       // pinned upload slots ("double buffering")
+constexpr int N_RES = 4;       // result ring
+
+struct Pipeline {
+    bool open = false;
+    int dtype = 0, mode = 0, host_result = 0;
+    size_t frame_bytes = 0, slot_bytes = 0, field_bytes = 0;
+    cudaStream_t s_copy = nullptr, s_comp = nullptr, s_down = nullptr;
+    void *pin[N_PIN] = {nullptr, nullptr};
+    void *raw[N_PIN] = {nullptr, nullptr};
+    float *res_dev[N_RES] = {};
+    float *res_host[N_RES] = {};
+    cudaEvent_t h2d_done[N_PIN] = {}, cvt_done[N_PIN] = {}, solve_done[N_RES] = {}, d2h_done[N_RES] = {};
+    bool cvt_rec[N_PIN] = {}, d2h_rec[N_RES] = {};
+    long long acquired = 0, submitted = 0, produced = 0, collected = 0;
+    int cur_slot = -1;
+};
+
+}  // namespace
+
+struct of_context {
+    int W, H, levels, R, iterations, window_type;
+    int device;
+    float eps_rel, max_step;
+    Level lv[OF_MAX_LEVELS];
+    float *pyr[N_PYR][OF_MAX_LEVELS];
+    float *u[OF_MAX_LEVELS], *v[OF_MAX_LEVELS];
+    float *S;
+    size_t plane;
+    float *det;
+    uint8_t *valid;
+    WinWeights ww;
+    bool use_graph;
+    std::vector<GraphEntry> graphs;
+    unsigned long long stamp;
+    int last_launches;
+    std::vector<void *> allocs;
+    Pipeline pipe;
+};
+
+namespace {
+
+inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
+
+template <int R> int setup_attrs()
+{
+    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K2Cfg<R>::SMEM));
+    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K3Cfg<R>::SMEM));
+    return OF_OK;
+}
+
+template <int R>
+void launch_k2(const of_context *c, int l, const float *I1, const float *I2, cudaStream_t st)
+{
+    const Level &L = c->lv[l];
+    dim3 grid((L.W + K2_TW - 1) / K2_TW, (L.H + K2_TH - 1) / K2_TH);
+    k2_products_hsum<R><<<grid, 256, K2Cfg<R>::SMEM, st>>>(I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, c->ww);
+}
+
+template <int R>
+void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, cudaStream_t st)
+{
+    const Level &L = c->lv[l];
+    dim3 grid((L.W + K3_TW - 1) / K3_TW, (L.H + K3_TH - 1) / K3_TH);
+    SolveParams sp = {0.5f * c->eps_rel, c->max_step};
+    k3_vsum_solve<R><<<grid, 256, K3Cfg<R>::SMEM, st>>>(c->S, c->plane, c->u[l], c->v[l], u_out, v_out, out_pitch,
+                                                        last ? c->valid : nullptr, last ? c->det : nullptr, L.W, L.H,
+                                                        L.pitch, c->ww, sp);
+}
+
+#define DISPATCH_R(R_, CALL)                                                                       \
+    switch (R_) {                                                                                  \
+    case 1: { constexpr int R = 1; CALL; } break;   case 2: { constexpr int R = 2; CALL; } break;   \
+    case 3: { constexpr int R = 3; CALL; } break;   case 4: { constexpr int R = 4; CALL; } break;   \
+    case 5: { constexpr int R = 5; CALL; } break;   case 6: { constexpr int R = 6; CALL; } break;   \
+    case 7: { constexpr int R = 7; CALL; } break;   case 8: { constexpr int R = 8; CALL; } break;   \
+    case 9: { constexpr int R = 9; CALL; } break;   case 10: { constexpr int R = 10; CALL; } break; \
+    case 11: { constexpr int R = 11; CALL; } break; case 12: { constexpr int R = 12; CALL; } break; \
+    case 13: { constexpr int R = 13; CALL; } break; case 14: { constexpr int R = 14; CALL; } break; \
+    case 15: { constexpr int R = 15; CALL; } break; case 16: { constexpr int R = 16; CALL; } break; \
+    default: break;                                                                                \
+    }
+
+void run_k2(const of_context *c, int l, const float *I1, const float *I2, cudaStream_t st)
+{
+    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, st));
+}
+void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, cudaStream_t st)
+{
+    DISPATCH_R(c->R, launch_k3<R>(c, l, u_out, v_out, out_pitch, last, st));
+}
+
+void run_convert(const of_context *c, int dtype, const void *a, const void *b, float *da, float *db, cudaStream_t st)
+{
+    const Level &L = c->lv[0];
+    dim3 grid((L.W + 1023) / 1024, L.H, b ? 2 : 1);
+    if (dtype == OF_DTYPE_U8)
+        k0_convert<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)a, (const uint8_t *)b, da, db, L.W, L.H, L.pitch);
+    else if (dtype == OF_DTYPE_U16)
+        k0_convert<uint16_t><<<grid, 256, 0, st>>>((const uint16_t *)a, (const uint16_t *)b, da, db, L.W, L.H, L.pitch);
+    else
+        k0_convert<float><<<grid, 256, 0, st>>>((const float *)a, (const float *)b, da, db, L.W, L.H, L.pitch);
+}
+
+void run_pyramid(const of_context *c, int l, const float *sa, const float *sb, float *da, float *db, cudaStream_t st)
+{
+    const Level &S = c->lv[l], &D = c->lv[l + 1];
+    dim3 grid((D.W + K1_TW - 1) / K1_TW, (D.H + K1_TH - 1) / K1_TH, sb ? 2 : 1);
+    k1_pyramid_down<<<grid, 256, 0, st>>>(sa, sb, da, db, S.W, S.H, S.pitch, D.W, D.H, D.pitch);
+}
+
+void run_upsample(const of_context *c, int l, cudaStream_t st)   // level l+1 -> l
+{
+    const Level &F = c->lv[l], &Cc = c->lv[l + 1];
+    dim3 grid((F.W + 63) / 64, (F.H + 3) / 4);
+    k4_upsample_flow<<<grid, 256, 0, st>>>(c->u[l + 1], c->v[l + 1], Cc.W, Cc.H, Cc.pitch, c->u[l], c->v[l], F.W, F.H, F.pitch);
+}
+
+// Enqueue the whole path of one Job (rows a1-a10).  Returns the number of kernels launched.
+int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
+{
+    int n = 0;
+    if (j.cvtA >= 0) {
+        const bool both = j.cvtB >= 0;
+        run_convert(c, j.dtype, j.rawA, both ? j.rawB : nullptr, c->pyr[j.cvtA][0], both ? c->pyr[j.cvtB][0] : nullptr, st);
+        ++n;
+        for (int l = 0; l + 1 < c->levels; ++l) {
+            run_pyramid(c, l, c->pyr[j.cvtA][l], both ? c->pyr[j.cvtB][l] : nullptr, c->pyr[j.cvtA][l + 1],
+                        both ? c->pyr[j.cvtB][l + 1] : nullptr, st);
+            ++n;
+        }
+    }
+    const int top = c->levels - 1;
+    cudaMemsetAsync(c->u[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
+    cudaMemsetAsync(c->v[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
+    for (int l = top; l >= 0; --l) {
+        if (l < top) { run_upsample(c, l, st); ++n; }
+        for (int it = 0; it < c->iterations; ++it) {
+            run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], st);
+            const bool last = (l == 0 && it == c->iterations - 1);
+            if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, st);
+            else run_k3(c, l, c->u[l], c->v[l], c->lv[l].pitch, false, st);
+            n += 2;
+        }
+    }
+    return n;
+}
+
+int submit_job(of_context *c, const Job &j, cudaStream_t st)
+{
+    CU_TRY(cudaSetDevice(c->device));
+    if (!c->use_graph || st == nullptr) {
+        c->last_launches = enqueue_job(c, j, st);
+        CU_TRY(cudaGetLastError());
+        return OF_OK;
+    }
+    ++c->stamp;
+    for (auto &g : c->graphs)
+        if (g.job == j) {
+            g.stamp = c->stamp;
+            CU_TRY(cudaGraphLaunch(g.exec, st));
+            c->last_launches = g.launches;
+            return OF_OK;
+        }
+    cudaGraph_t graph = nullptr;
+    CU_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+    int n = enqueue_job(c, j, st);
+    cudaError_t e1 = cudaGetLastError();
+    cudaError_t e2 = cudaStreamEndCapture(st, &graph);
+    if (e1 != cudaSuccess || e2 != cudaSuccess || graph == nullptr) {
+        if (graph) cudaGraphDestroy(graph);
+        return fail(OF_ERR_CUDA, "graph capture failed: %s / %s", cudaGetErrorString(e1), cudaGetErrorString(e2));
+    }
+    cudaGraphExec_t exec = nullptr;
+    cudaError_t e3 = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e3 != cudaSuccess) return fail(OF_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e3));
+    if (c->graphs.size() >= 8) {
+        size_t old = 0;
+        for (size_t i = 1; i < c->graphs.size(); ++i)
+            if (c->graphs[i].stamp < c->graphs[old].stamp) old = i;
+        cudaGraphExecDestroy(c->graphs[old].exec);
+        c->graphs.erase(c->graphs.begin() + old);
+    }
+    c->graphs.push_back({j, exec, c->stamp, n});
+    CU_TRY(cudaGraphLaunch(exec, st));
+    c->last_launches = n;
+    return OF_OK;
+}
+
+void drop_graphs(of_context *c)
+{
+    for (auto &g : c->graphs) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+}
+
+int dev_alloc(of_context *c, void **p, size_t bytes)
+{
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) return fail(OF_ERR_ALLOC, "cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+    c->allocs.push_back(*p);
+    return OF_OK;
+}
+
+int compute_any(of_handle h, int dtype, const void *I1, const void *I2, float *u, float *v, void *stream)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    if (!I1 || !I2 || !u || !v) return fail(OF_ERR_INVALID_ARG, "null image or field pointer");
+    if (h->pipe.open) return fail(OF_ERR_STATE, "handle is in streaming mode; call of_stream_close first");
+    Job j;
+    memset(&j, 0, sizeof j);
+    j.dtype = dtype; j.rawA = I1; j.rawB = I2; j.cvtA = 0; j.cvtB = 1; j.s1 = 0; j.s2 = 1; j.u_out = u; j.v_out = v;
+    return submit_job(h, j, (cudaStream_t)stream);
+}
+
+int copy_plane_dense(const float *src, int pitch, int W, int H, float *dst, cudaStream_t st)
+{
+    CU_TRY(cudaMemcpy2DAsync(dst, sizeof(float) * W, src, sizeof(float) * pitch, sizeof(float) * W, H,
+                             cudaMemcpyDeviceToDevice, st));
+    return OF_OK;
+}
+
+void pipe_release(of_context *c)
+{
+    Pipeline &p = c->pipe;
+    if (p.s_copy) cudaStreamSynchronize(p.s_copy);
+    if (p.s_comp) cudaStreamSynchronize(p.s_comp);
+    if (p.s_down) cudaStreamSynchronize(p.s_down);
+    for (int i = 0; i < N_PIN; ++i) {
+        if (p.pin[i]) cudaFreeHost(p.pin[i]);
+        if (p.raw[i]) cudaFree(p.raw[i]);
+        if (p.h2d_done[i]) cudaEventDestroy(p.h2d_done[i]);
+        if (p.cvt_done[i]) cudaEventDestroy(p.cvt_done[i]);
+    }
+    for (int i = 0; i < N_RES; ++i) {
+        if (p.res_dev[i]) cudaFree(p.res_dev[i]);
+        if (p.res_host[i]) cudaFreeHost(p.res_host[i]);
+        if (p.solve_done[i]) cudaEventDestroy(p.solve_done[i]);
+        if (p.d2h_done[i]) cudaEventDestroy(p.d2h_done[i]);
+    }
+    if (p.s_copy) cudaStreamDestroy(p.s_copy);
+    if (p.s_comp) cudaStreamDestroy(p.s_comp);
+    if (p.s_down) cudaStreamDestroy(p.s_down);
+    p = Pipeline();
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+const char *of_last_error(void) { return g_err.c_str(); }
+
+of_handle of_create(int width, int height, int levels, int window_radius, int iterations, int window_type)
+{
+    g_err.clear();
+    if (width < 1 || height < 1 || width > (1 << 15) || height > (1 << 15)) { fail(OF_ERR_INVALID_ARG, "bad image size %dx%d", width, height); return nullptr; }
+    if (levels < 1 || levels > OF_MAX_LEVELS) { fail(OF_ERR_INVALID_ARG, "levels must be in [1,%d]", OF_MAX_LEVELS); return nullptr; }
+    if (window_radius < 1 || window_radius > OF_MAX_WINDOW_RADIUS) { fail(OF_ERR_INVALID_ARG, "window_radius must be in [1,%d]", OF_MAX_WINDOW_RADIUS); return nullptr; }
+    if (iterations < 1) { fail(OF_ERR_INVALID_ARG, "iterations must be >= 1"); return nullptr; }
+    if (window_type != OF_WINDOW_BOX && window_type != OF_WINDOW_GAUSSIAN) { fail(OF_ERR_INVALID_ARG, "unknown window_type %d", window_type); return nullptr; }
+    Level lv[OF_MAX_LEVELS];
+    lv[0] = {width, height, round_up(width, 32)};
+    for (int l = 1; l < levels; ++l) {
+        lv[l].W = (lv[l - 1].W + 1) / 2;
+        lv[l].H = (lv[l - 1].H + 1) / 2;
+        lv[l].pitch = round_up(lv[l].W, 32);
+    }
+    if (lv[levels - 1].W < 2 * window_radius + 1 || lv[levels - 1].H < 2 * window_radius + 1) {
+        fail(OF_ERR_INVALID_ARG, "coarsest level %dx%d is smaller than the window (%d)", lv[levels - 1].W, lv[levels - 1].H, 2 * window_radius + 1);
+        return nullptr;
+    }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { fail(OF_ERR_CUDA, "no usable CUDA device: %s", cudaGetErrorString(e)); return nullptr; }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) { fail(OF_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)); return nullptr; }
+    if (prop.major != 10) { fail(OF_ERR_CUDA, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor); return nullptr; }
+
+    of_context *c = new (std::nothrow) of_context();
+    if (!c) { fail(OF_ERR_ALLOC, "out of host memory"); return nullptr; }
+    c->W = width; c->H = height; c->levels = levels; c->R = window_radius; c->iterations = iterations;
+    c->window_type = window_type; c->device = dev; c->eps_rel = 1e-3f; c->max_step = 3.0f;
+    c->use_graph = true; c->stamp = 0; c->last_launches = 0;
+    memcpy(c->lv, lv, sizeof lv);
+    memset(&c->ww, 0, sizeof c->ww);
+    for (int t = -window_radius; t <= window_radius; ++t) {
+        double w = 1.0;
+        if (window_type == OF_WINDOW_GAUSSIAN) {
+            double sigma = (double)window_radius / 3.0;
+            w = std::exp(-(double)(t * t) / (2.0 * sigma * sigma));
+        }
+        c->ww.w[t + window_radius] = (float)w;
+    }
+    int rc = OF_OK;
+    for (int l = 0; l < levels && rc == OF_OK; ++l) {
+        size_t bytes = sizeof(float) * (size_t)lv[l].pitch * lv[l].H;
+        for (int s = 0; s < N_PYR && rc == OF_OK; ++s) rc = dev_alloc(c, (void **)&c->pyr[s][l], bytes);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->u[l], bytes);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->v[l], bytes);
+    }
+    c->plane = (size_t)lv[0].pitch * lv[0].H;
+    if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->S, sizeof(float) * 5 * c->plane);
+    if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->det, sizeof(float) * c->plane);
+    if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->valid, (size_t)width * height);
+    if (rc == OF_OK) {
+        // padding columns of every plane must hold finite values (they are read, never used)
+        for (void *p : c->allocs) (void)p;
+        for (int l = 0; l < levels; ++l) {
+            size_t bytes = sizeof(float) * (size_t)lv[l].pitch * lv[l].H;
+            for (int s = 0; s < N_PYR; ++s) cudaMemset(c->pyr[s][l], 0, bytes);
+            cudaMemset(c->u[l], 0, bytes);
+            cudaMemset(c->v[l], 0, bytes);
+        }
+        cudaMemset(c->S, 0, sizeof(float) * 5 * c->plane);
+        cudaMemset(c->det, 0, sizeof(float) * c->plane);
+        cudaMemset(c->valid, 0, (size_t)width * height);
+        if (cudaDeviceSynchronize() != cudaSuccess) rc = fail(OF_ERR_CUDA, "memset failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    if (rc == OF_OK) { DISPATCH_R(window_radius, rc = setup_attrs<R>()); }
+    if (rc != OF_OK) { std::string keep = g_err; of_destroy(c); g_err = keep; return nullptr; }
+    return c;
+}
+
+void of_destroy(of_handle h)
+{
+    if (!h) return;
+    cudaSetDevice(h->device);
+    if (h->pipe.open) pipe_release(h);
+    cudaDeviceSynchronize();
+    drop_graphs(h);
+    for (void *p : h->allocs) cudaFree(p);
+    delete h;
+}
+
+int of_compute(of_handle h, const float *I1, const float *I2, float *u, float *v, void *stream)
+{
+    return compute_any(h, OF_DTYPE_F32, I1, I2, u, v, stream);
+}
+int of_compute_u8(of_handle h, const uint8_t *I1, const uint8_t *I2, float *u, float *v, void *stream)
+{
+    return compute_any(h, OF_DTYPE_U8, I1, I2, u, v, stream);
+}
+int of_compute_u16(of_handle h, const uint16_t *I1, const uint16_t *I2, float *u, float *v, void *stream)
+{
+    return compute_any(h, OF_DTYPE_U16, I1, I2, u, v, stream);
+}
+
+int of_set_conditioning(of_handle h, float eps_rel, float max_step_px)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    if (!(eps_rel >= 0.f) || !(max_step_px > 0.f)) return fail(OF_ERR_INVALID_ARG, "eps_rel must be >= 0 and max_step_px > 0");
+    h->eps_rel = eps_rel;
+    h->max_step = max_step_px;
+    drop_graphs(h);
+    return OF_OK;
+}
+
+int of_set_graph(of_handle h, int enable)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    h->use_graph = enable != 0;
+    if (!h->use_graph) drop_graphs(h);
+    return OF_OK;
+}
+
+int of_get_validity(of_handle h, uint8_t *mask_dev, void *stream)
+{
+    if (!h || !mask_dev) return fail(OF_ERR_INVALID_ARG, "null argument");
+    CU_TRY(cudaMemcpyAsync(mask_dev, h->valid, (size_t)h->W * h->H, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return OF_OK;
+}
+
+int of_level_size(of_handle h, int level, int *width, int *height)
+{
+    if (!h || level < 0 || level >= h->levels) return fail(OF_ERR_INVALID_ARG, "bad level");
+    if (width) *width = h->lv[level].W;
+    if (height) *height = h->lv[level].H;
+    return OF_OK;
+}
+
+int of_last_launch_count(of_handle h) { return h ? h->last_launches : fail(OF_ERR_INVALID_ARG, "null handle"); }
+
+int of_get_debug_plane(of_handle h, int level, int which, float *out_dev, void *stream)
+{
+    if (!h || !out_dev || level < 0 || level >= h->levels) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    const Level &L = h->lv[level];
+    const float *src = nullptr;
+    if (which == 0) src = h->pyr[0][level];
+    else if (which == 1) src = h->pyr[1][level];
+    else if (which == 2) src = h->u[level];
+    else if (which == 3) src = h->v[level];
+    else if (which >= 4 && which <= 8) src = h->S + (size_t)(which - 4) * h->plane;
+    else if (which == 9 && level == 0) src = h->det;
+    else return fail(OF_ERR_INVALID_ARG, "bad plane selector %d", which);
+    return copy_plane_dense(src, L.pitch, L.W, L.H, out_dev, (cudaStream_t)stream);
+}
+
+int of_run_step(of_handle h, int level, int which, void *stream)
+{
+    if (!h || level < 0 || level >= h->levels || which < 0 || which > 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    CU_TRY(cudaSetDevice(h->device));
+    if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], (cudaStream_t)stream);
+    else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, (cudaStream_t)stream);
+    CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+int of_pyramid_down(const float *src, int width, int height, float *dst, void *stream)
+{
+    if (!src || !dst || width < 1 || height < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    int Wd = (width + 1) / 2, Hd = (height + 1) / 2;
+    dim3 grid((Wd + K1_TW - 1) / K1_TW, (Hd + K1_TH - 1) / K1_TH, 1);
+    k1_pyramid_down<<<grid, 256, 0, (cudaStream_t)stream>>>(src, nullptr, dst, nullptr, width, height, width, Wd, Hd, Wd);
+    CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+int of_upsample_flow(const float *uc, const float *vc, int wc, int hc, float *u, float *v, int width, int height, void *stream)
+{
+    if (!uc || !vc || !u || !v || wc < 1 || hc < 1 || width < 1 || height < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    if (wc != (width + 1) / 2 || hc != (height + 1) / 2) return fail(OF_ERR_INVALID_ARG, "coarse size must be ((W+1)/2,(H+1)/2)");
+    dim3 grid((width + 63) / 64, (height + 3) / 4);
+    k4_upsample_flow<<<grid, 256, 0, (cudaStream_t)stream>>>(uc, vc, wc, hc, wc, u, v, width, height, width);
+    CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// frame pipeline (row a11)
+// ------------------------------------------------------------------------------------------------
+int of_stream_open(of_handle h, int dtype, int mode, int result_on_host)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    if (h->pipe.open) return fail(OF_ERR_STATE, "pipeline already open");
+    if (dtype < OF_DTYPE_F32 || dtype > OF_DTYPE_U16) return fail(OF_ERR_INVALID_ARG, "bad dtype");
+    if (mode != OF_STREAM_CONSECUTIVE && mode != OF_STREAM_PAIRS) return fail(OF_ERR_INVALID_ARG, "bad mode");
+    CU_TRY(cudaSetDevice(h->device));
+    Pipeline &p = h->pipe;
+    p = Pipeline();
+    p.dtype = dtype; p.mode = mode; p.host_result = result_on_host ? 1 : 0;
+    size_t es = dtype == OF_DTYPE_U8 ? 1 : (dtype == OF_DTYPE_U16 ? 2 : 4);
+    p.frame_bytes = es * (size_t)h->W * h->H;
+    p.slot_bytes = p.frame_bytes * (mode == OF_STREAM_PAIRS ? 2 : 1);
+    p.field_bytes = sizeof(float) * (size_t)h->W * h->H;
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return r == cudaSuccess; };
+    ok(cudaStreamCreateWithFlags(&p.s_copy, cudaStreamNonBlocking));
+    ok(cudaStreamCreateWithFlags(&p.s_comp, cudaStreamNonBlocking));
+    ok(cudaStreamCreateWithFlags(&p.s_down, cudaStreamNonBlocking));
+    for (int i = 0; i < N_PIN; ++i) {
+        ok(cudaHostAlloc(&p.pin[i], p.slot_bytes, cudaHostAllocDefault));
+        ok(cudaMalloc(&p.raw[i], p.slot_bytes));
+        ok(cudaEventCreateWithFlags(&p.h2d_done[i], cudaEventDisableTiming));
+        ok(cudaEventCreateWithFlags(&p.cvt_done[i], cudaEventDisableTiming));
+    }
+    for (int i = 0; i < N_RES; ++i) {
+        ok(cudaMalloc((void **)&p.res_dev[i], 2 * p.field_bytes));
+        if (p.host_result) ok(cudaHostAlloc((void **)&p.res_host[i], 2 * p.field_bytes, cudaHostAllocDefault));
+        ok(cudaEventCreateWithFlags(&p.solve_done[i], cudaEventDisableTiming));
+        ok(cudaEventCreateWithFlags(&p.d2h_done[i], cudaEventDisableTiming));
+    }
+    if (e != cudaSuccess) {
+        pipe_release(h);
+        return fail(e == cudaErrorMemoryAllocation ? OF_ERR_ALLOC : OF_ERR_CUDA, "of_stream_open: %s", cudaGetErrorString(e));
+    }
+    p.open = true;
+    return OF_OK;
+}
+
+void *of_stream_acquire(of_handle h)
+{
+    if (!h || !h->pipe.open) { fail(OF_ERR_STATE, "pipeline not open"); return nullptr; }
+    Pipeline &p = h->pipe;
+    if (p.cur_slot >= 0) return p.pin[p.cur_slot];          // acquired but not yet submitted
+    int s = (int)(p.acquired % N_PIN);
+    if (p.acquired >= N_PIN) {
+        cudaError_t e = cudaEventSynchronize(p.h2d_done[s]);
+        if (e != cudaSuccess) { fail(OF_ERR_CUDA, "cudaEventSynchronize: %s", cudaGetErrorString(e)); return nullptr; }
+    }
+    p.cur_slot = s;
+    ++p.acquired;
+    return p.pin[s];
+}
+
+int of_stream_submit(of_handle h)
+{
+    if (!h || !h->pipe.open) return fail(OF_ERR_STATE, "pipeline not open");
+    Pipeline &p = h->pipe;
+    if (p.cur_slot < 0) return fail(OF_ERR_STATE, "of_stream_submit without of_stream_acquire");
+    const bool yields = (p.mode == OF_STREAM_PAIRS) || p.submitted >= 1;
+    if (yields && p.produced - p.collected >= 2)
+        return fail(OF_ERR_STATE, "two fields are waiting: call of_stream_result before submitting more");
+    CU_TRY(cudaSetDevice(h->device));
+    const int s = p.cur_slot;
+    // upload: the device slot must have been consumed by the conversion of the frame it held before
+    if (p.cvt_rec[s]) CU_TRY(cudaStreamWaitEvent(p.s_copy, p.cvt_done[s], 0));
+    CU_TRY(cudaMemcpyAsync(p.raw[s], p.pin[s], p.slot_bytes, cudaMemcpyHostToDevice, p.s_copy));
+    CU_TRY(cudaEventRecord(p.h2d_done[s], p.s_copy));
+    CU_TRY(cudaStreamWaitEvent(p.s_comp, p.h2d_done[s], 0));
+
+    Job j;
+    memset(&j, 0, sizeof j);
+    j.dtype = p.dtype;
+    const int r = (int)(p.produced % N_RES);
+    if (p.mode == OF_STREAM_PAIRS) {
+        j.rawA = p.raw[s]; j.rawB = (const char *)p.raw[s] + p.frame_bytes; j.cvtA = 0; j.cvtB = 1; j.s1 = 0; j.s2 = 1;
+    } else {
+        const int ps = (int)(p.submitted % N_PYR);
+        j.rawA = p.raw[s]; j.rawB = nullptr; j.cvtA = ps; j.cvtB = -1; j.s1 = 1 - ps; j.s2 = ps;
+    }
+    if (yields) {
+        if (p.d2h_rec[r]) CU_TRY(cudaStreamWaitEvent(p.s_comp, p.d2h_done[r], 0));
+        j.u_out = p.res_dev[r];
+        j.v_out = p.res_dev[r] + (size_t)h->W * h->H;
+        int rc = submit_job(h, j, p.s_comp);
+        if (rc != OF_OK) return rc;
+        CU_TRY(cudaEventRecord(p.cvt_done[s], p.s_comp));   // (recorded after the solve: conservative)
+        p.cvt_rec[s] = true;
+        CU_TRY(cudaEventRecord(p.solve_done[r], p.s_comp));
+        if (p.host_result) {
+            CU_TRY(cudaStreamWaitEvent(p.s_down, p.solve_done[r], 0));
+            CU_TRY(cudaMemcpyAsync(p.res_host[r], p.res_dev[r], 2 * p.field_bytes, cudaMemcpyDeviceToHost, p.s_down));
+            CU_TRY(cudaEventRecord(p.d2h_done[r], p.s_down));
+            p.d2h_rec[r] = true;
+        }
+        ++p.produced;
+    } else {
+        // first frame of a consecutive stream: convert + pyramid only
+        const int ps = (int)(p.submitted % N_PYR);
+        run_convert(h, p.dtype, p.raw[s], nullptr, h->pyr[ps][0], nullptr, p.s_comp);
+        for (int l = 0; l + 1 < h->levels; ++l) run_pyramid(h, l, h->pyr[ps][l], nullptr, h->pyr[ps][l + 1], nullptr, p.s_comp);
+        CU_TRY(cudaGetLastError());
+        CU_TRY(cudaEventRecord(p.cvt_done[s], p.s_comp));
+        p.cvt_rec[s] = true;
+        h->last_launches = h->levels;
+    }
+    ++p.submitted;
+    p.cur_slot = -1;
+    return OF_OK;
+}
+
+int of_stream_result(of_handle h, const float **u, const float **v, int *pair_index)
+{
+    if (!h || !h->pipe.open) return fail(OF_ERR_STATE, "pipeline not open");
+    Pipeline &p = h->pipe;
+    if (p.collected >= p.produced) return fail(OF_ERR_STATE, "no field pending");
+    const int r = (int)(p.collected % N_RES);
+    CU_TRY(cudaEventSynchronize(p.host_result ? p.d2h_done[r] : p.solve_done[r]));
+    const float *base = p.host_result ? p.res_host[r] : p.res_dev[r];
+    if (u) *u = base;
+    if (v) *v = base + (size_t)h->W * h->H;
+    if (pair_index) *pair_index = (int)p.collected;
+    ++p.collected;
+    return OF_OK;
+}
+
+int of_stream_close(of_handle h)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    if (!h->pipe.open) return OF_OK;
+    cudaSetDevice(h->device);
+    pipe_release(h);
+    drop_graphs(h);
+    return OF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,331 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by element,
+on the same seeded inputs.  Run on the B200 box with `pytest -m gpu`.
+
+Tolerance (BASELINE.json:5, D23): max <= 1e-3 px, RMS <= 1e-4 px on pixels whose determinant exceeds
+1e-3 of the field maximum; identical validity masks everywhere.
+"""
+import numpy as np
+import pytest
+
+from paper_1306_2461_b200 import synthetic as syn
+from parity import assert_parity, compare_flow
+
+pytestmark = pytest.mark.gpu
+
+BOX, GAUSS = 0, 1
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    return t
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1306_2461_b200 import binding
+    binding.lib()          # fails loudly if liboptflow.so is missing
+    return binding
+
+
+def gpu_solve(torch, B, I1, I2, levels, R, iters, wt, as_float=False, graph=True):
+    H, W = I1.shape
+    with B.OpticalFlow(W, H, levels, R, iters, wt) as of:
+        of.set_graph(graph)
+        if as_float:
+            d1 = torch.from_numpy(I1.astype(np.float32)).cuda()
+            d2 = torch.from_numpy(I2.astype(np.float32)).cuda()
+        elif I1.dtype == np.uint16:
+            d1 = torch.from_numpy(I1.view(np.int16)).cuda()
+            d2 = torch.from_numpy(I2.view(np.int16)).cuda()
+        else:
+            d1 = torch.from_numpy(I1).cuda()
+            d2 = torch.from_numpy(I2).cuda()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            u, v = of.compute(d1, d2)
+            m = of.validity()
+        s.synchronize()
+        return u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy(), of.last_launch_count()
+
+
+def run_case(torch, B, oracle, c, as_float=False):
+    ref = oracle.solve(c.I1, c.I2, c.levels, c.window_radius, c.iterations, c.window_type)
+    u, v, m, n = gpu_solve(torch, B, c.I1, c.I2, c.levels, c.window_radius, c.iterations, c.window_type, as_float)
+    st = assert_parity(u, v, m, ref, c.name)
+    print(c.name, c.width, c.height, st, "launches", n)
+    return st
+
+
+# ---------------------------------------------------------------------------- the five configs
+def test_config1_256_uniform_shift(torch, B, oracle):
+    """BASELINE.json:7: fp32-from-uint8, 1 level, box R 8, 4 iterations; expected flow (1.3,-0.7)."""
+    c = syn.config1()
+    run_case(torch, B, oracle, c, as_float=True)
+    u, v, m, _ = gpu_solve(torch, B, c.I1, c.I2, 1, 8, 4, BOX, as_float=True)
+    assert abs(np.median(u) - 1.3) < 0.05 and abs(np.median(v) + 0.7) < 0.05
+
+
+def test_config2_small_ragged(torch, B, oracle):
+    """config-2 statistics at a size that is no multiple of any tile (several tiles + ragged tail)."""
+    run_case(torch, B, oracle, syn.config2(330, 214))
+
+
+def test_config2_1024_vortex(torch, B, oracle):
+    run_case(torch, B, oracle, syn.config2())
+
+
+def test_config3_small_gaussian(torch, B, oracle):
+    run_case(torch, B, oracle, syn.config3(400, 296))
+
+
+def test_config3_1280x1024_gaussian(torch, B, oracle):
+    """BASELINE.json:9 -- the bench workload, in the launch configuration bench.py times."""
+    run_case(torch, B, oracle, syn.config3())
+
+
+def test_config4_small_u16(torch, B, oracle):
+    run_case(torch, B, oracle, syn.config4(400, 360, filt_sigma=48.0))
+
+
+def test_config4_2048_u16(torch, B, oracle):
+    run_case(torch, B, oracle, syn.config4())
+
+
+def test_config5_streaming(torch, B, oracle):
+    """BASELINE.json:11: consecutive frames through the pinned double-buffered pipeline.  Every field
+    must equal (bitwise) the non-streaming call on the same pair; sampled pairs are checked against
+    the oracle."""
+    import os
+    n_frames = int(os.environ.get("OF_TEST_STREAM_FRAMES", "256"))
+    st = syn.Config5Stream(n_frames)
+    W, H = st.width, st.height
+    sample = sorted({0, (n_frames - 1) // 2, n_frames - 2})
+    frames_kept = {}
+    fields = {}
+    with B.OpticalFlow(*st.create_args) as of, B.OpticalFlow(*st.create_args) as of2:
+        of.stream_open(B.OF_DTYPE_U8, B.OF_STREAM_CONSECUTIVE, True)
+        prev = None
+        submitted = 0
+        for k, f in enumerate(st.frames()):
+            slot = of.stream_acquire()
+            slot[...] = f
+            of.stream_submit()
+            submitted += 1
+            if k >= 1:
+                if (k - 1) in sample:
+                    frames_kept[k - 1] = (prev.copy(), f.copy())
+                # stay one field behind so upload k+1 overlaps solve k
+                if k >= 2:
+                    idx, u, v = of.stream_result()
+                    assert idx == k - 2
+                    if idx in sample or idx % 37 == 0:
+                        fields[idx] = (u.copy(), v.copy())
+            prev = f
+        idx, u, v = of.stream_result()
+        assert idx == n_frames - 2
+        fields[idx] = (u.copy(), v.copy())
+        of.stream_close()
+        # non-streaming call on the kept pairs must agree bitwise; oracle parity on them
+        for idx, (f1, f2) in frames_kept.items():
+            d1, d2 = torch.from_numpy(f1).cuda(), torch.from_numpy(f2).cuda()
+            u2, v2 = of2.compute(d1, d2)
+            m2 = of2.validity()
+            torch.cuda.synchronize()
+            assert np.array_equal(u2.cpu().numpy(), fields[idx][0]), idx
+            assert np.array_equal(v2.cpu().numpy(), fields[idx][1]), idx
+            ref = oracle.solve(f1, f2, st.levels, st.window_radius, st.iterations, st.window_type)
+            print("config5 pair", idx, assert_parity(fields[idx][0], fields[idx][1], m2.cpu().numpy(), ref, "config5"))
+    # the convected shear layer moves right at ~2+-3 px/frame: sanity on the sign of the field
+    u_last = fields[n_frames - 2][0]
+    assert u_last[: H // 4].mean() > 3.0 and u_last[-H // 4:].mean() < 0.5
+
+
+def test_stream_pairs_mode(torch, B, oracle):
+    c = syn.config2(320, 256)
+    ref = oracle.solve(c.I1, c.I2, c.levels, c.window_radius, c.iterations, c.window_type)
+    with B.OpticalFlow(*c.create_args) as of:
+        of.stream_open(B.OF_DTYPE_U8, B.OF_STREAM_PAIRS, True)
+        for rep in range(5):
+            slot = of.stream_acquire()
+            slot[0] = c.I1
+            slot[1] = c.I2
+            of.stream_submit()
+            idx, u, v = of.stream_result()
+            assert idx == rep
+            assert_parity(u, v, None, ref, "pairs-mode")
+        # overflow protection: a third uncollected field is refused
+        for rep in range(2):
+            slot = of.stream_acquire(); slot[0] = c.I1; slot[1] = c.I2; of.stream_submit()
+        of.stream_acquire()
+        with pytest.raises(B.OptflowError):
+            of.stream_submit()
+        of.stream_close()
+
+
+# ---------------------------------------------------------------------------- single steps
+def test_pyramid_step_matches_oracle(torch, B, oracle):
+    rng = np.random.default_rng(1)
+    for (H, W) in ((64, 64), (37, 131), (5, 9), (1024, 1280)):
+        img = rng.integers(0, 4096, (H, W)).astype(np.float32)
+        ref = oracle.downsample(img)
+        out = B.pyramid_down(torch.from_numpy(img).cuda()).cpu().numpy()
+        assert out.shape == ref.shape
+        assert np.max(np.abs(out - ref)) <= 1e-6 * 4096, (H, W)
+        # integers < 2^12 with dyadic taps: one level is exact in fp32
+        assert np.array_equal(out.astype(np.float64), ref), (H, W)
+
+
+def test_upsample_step_matches_oracle(torch, B, oracle):
+    rng = np.random.default_rng(2)
+    for (H, W) in ((64, 64), (37, 131), (7, 10)):
+        hc, wc = (H + 1) // 2, (W + 1) // 2
+        uc = rng.uniform(-8, 8, (hc, wc)).astype(np.float32)
+        vc = rng.uniform(-8, 8, (hc, wc)).astype(np.float32)
+        u, v = B.upsample_flow(torch.from_numpy(uc).cuda(), torch.from_numpy(vc).cuda(), W, H)
+        assert np.max(np.abs(u.cpu().numpy() - oracle.upsample_flow(uc, W, H))) < 2e-6
+        assert np.max(np.abs(v.cpu().numpy() - oracle.upsample_flow(vc, W, H))) < 2e-6
+
+
+def test_intermediates_per_level(torch, B, oracle):
+    """Pyramid levels, the per-level fields and det against the oracle's intermediates."""
+    c = syn.config3(352, 288)
+    ref = oracle.solve(c.I1, c.I2, 3, 6, 3, GAUSS, return_levels=True)
+    with B.OpticalFlow(352, 288, 3, 6, 3, GAUSS) as of:
+        u, v = of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda())
+        torch.cuda.synchronize()
+        P = c.I1.astype(np.float64)
+        for l in range(3):
+            g = of.debug_plane(l, 0).cpu().numpy()
+            assert np.max(np.abs(g - P)) < 1e-4, l
+            if l >= 1:
+                gu = of.debug_plane(l, 2).cpu().numpy()
+                S = np.ones_like(gu, dtype=bool)
+                assert np.sqrt(np.mean((gu - ref["level_u"][l]) ** 2)) < 1e-3, l
+            P = oracle.downsample(P)
+        det = of.debug_plane(0, 9).cpu().numpy()
+        assert np.max(np.abs(det - ref["det"])) <= 1e-4 * ref["det"].max()
+
+
+def test_single_iteration_kernels_vs_oracle(torch, B, oracle):
+    """K2 then K3 run once through of_run_step from a non-zero field equal one oracle iteration."""
+    c = syn.config1(192, 160)
+    I1, I2 = c.I1.astype(np.float64), c.I2.astype(np.float64)
+    with B.OpticalFlow(192, 160, 1, 8, 2, BOX) as of:
+        of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda())
+        torch.cuda.synchronize()
+        u0 = of.debug_plane(0, 2).cpu().numpy().astype(np.float64)    # field after iteration 1
+        v0 = of.debug_plane(0, 3).cpu().numpy().astype(np.float64)
+        of.run_step(0, 0)
+        of.run_step(0, 1)
+        torch.cuda.synchronize()
+        u1 = of.debug_plane(0, 2).cpu().numpy()
+        v1 = of.debug_plane(0, 3).cpu().numpy()
+    ru, rv, sums, valid, det = oracle.iteration(I1, I2, u0, v0, 8, BOX)
+    S = det > 1e-3 * det.max()
+    assert np.max(np.abs(u1 - ru)[S]) < 1e-4 and np.max(np.abs(v1 - rv)[S]) < 1e-4
+
+
+# ---------------------------------------------------------------------------- edge cases
+@pytest.mark.parametrize("W,H,L,R,it,wt", [
+    (17, 17, 1, 8, 2, BOX),          # image == window
+    (3, 3, 1, 1, 1, BOX),            # smallest legal
+    (33, 65, 1, 16, 3, GAUSS),       # maximum radius
+    (130, 70, 2, 4, 3, BOX),         # ragged, two levels, odd sizes downstream (65x35)
+    (129, 67, 3, 2, 2, GAUSS),       # odd sizes at every level
+    (1000, 36, 1, 1, 5, BOX),        # wide and flat
+    (36, 1000, 2, 5, 2, BOX),        # tall and thin
+])
+def test_ragged_and_degenerate_sizes(torch, B, oracle, W, H, L, R, it, wt):
+    rng = np.random.default_rng(W * 1000 + H)
+    xp, yp, amp = syn.seed_particles(rng, W, H, 0.05, 100, 255)
+    I1 = syn.quantize(syn.render_particles(xp, yp, amp, 1.2, W, H), np.uint8, 255)
+    I2 = syn.quantize(syn.render_particles(xp + 0.6, yp - 0.4, amp, 1.2, W, H), np.uint8, 255)
+    ref = oracle.solve(I1, I2, L, R, it, wt)
+    u, v, m, _ = gpu_solve(torch, B, I1, I2, L, R, it, wt)
+    if ref["det"].max() > 0:
+        assert_parity(u, v, m, ref, (W, H, L, R))
+    else:
+        assert np.array_equal(m, ref["valid"])
+
+
+def test_identical_images_exact_zero(torch, B):
+    c = syn.config2(300, 200)
+    u, v, m, _ = gpu_solve(torch, B, c.I1, c.I1, 2, 7, 4, BOX)
+    assert np.all(u == 0.0) and np.all(v == 0.0)
+
+
+def test_empty_images_all_invalid(torch, B, oracle):
+    z = np.zeros((96, 128), dtype=np.uint8)
+    u, v, m, _ = gpu_solve(torch, B, z, z, 2, 5, 2, BOX)
+    assert np.all(u == 0) and np.all(v == 0) and np.all(m == 0)
+    # sparse texture: most windows are empty -> masks must still agree exactly
+    z1, z2 = z.copy(), z.copy()
+    z1[40:44, 60:64] = 200
+    z2[40:44, 61:65] = 200
+    ref = oracle.solve(z1, z2, 1, 5, 3, BOX)
+    u, v, m, _ = gpu_solve(torch, B, z1, z2, 1, 5, 3, BOX)
+    assert np.array_equal(m, ref["valid"]) and 0 < m.sum() < m.size
+    assert np.all(u[m == 0] == 0)
+
+
+def test_saturated_and_large_displacements_stay_finite(torch, B, oracle):
+    """Full-scale 16-bit values and displacements far beyond eq. 1's range: finite, clamped to
+    +-3 px per iteration (D15), identical masks."""
+    rng = np.random.default_rng(5)
+    I1 = rng.integers(0, 65536, (120, 160)).astype(np.uint16)
+    I2 = np.roll(I1, 25, axis=1)
+    ref = oracle.solve(I1, I2, 1, 6, 4, BOX)
+    u, v, m, _ = gpu_solve(torch, B, I1, I2, 1, 6, 4, BOX)
+    assert np.isfinite(u).all() and np.isfinite(v).all()
+    assert np.abs(u).max() <= 12.0 + 1e-4 and np.abs(v).max() <= 12.0 + 1e-4
+    assert np.array_equal(m, ref["valid"])
+
+
+def test_graph_and_plain_launches_agree_bitwise_and_repeat(torch, B):
+    c = syn.config3(320, 256)
+    a = gpu_solve(torch, B, c.I1, c.I2, 3, 12, 4, GAUSS, graph=True)
+    b = gpu_solve(torch, B, c.I1, c.I2, 3, 12, 4, GAUSS, graph=False)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    assert a[3] == b[3] == 1 + 2 + 2 + 3 * 4 * 2          # convert, 2 pyramid steps, 2 upsamples, 24 iteration kernels
+    H, W = c.I1.shape
+    with B.OpticalFlow(W, H, 3, 12, 4, GAUSS) as of:
+        d1, d2 = torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            u1, v1 = of.compute(d1, d2)
+            u1 = u1.clone()
+            u2, v2 = of.compute(d1, d2)      # graph replay with new output pointers
+            u3, v3 = of.compute(d1, d2, u2, v2)   # same pointers: cached graph
+        s.synchronize()
+        assert torch.equal(u1, u2) and torch.equal(u1, u3) and np.array_equal(u1.cpu().numpy(), a[0])
+
+
+def test_large_image_crop_parity(torch, B, oracle):
+    """4096x3072, one level: the result in a window depends only on a neighbourhood of radius
+    iterations*(R+max|u|+2), so the oracle on a crop pins sampled outputs of the full-size run."""
+    W, H, R, it = 4096, 3072, 8, 3
+    rng = np.random.default_rng(77)
+    xp, yp, amp = syn.seed_particles(rng, W, H, 0.03, 150, 255)
+    I1 = syn.quantize(syn.render_particles(xp, yp, amp, 1.2, W, H), np.uint8, 255)
+    I2 = syn.quantize(syn.render_particles(xp + 1.4, yp + 0.8, amp, 1.2, W, H), np.uint8, 255)
+    u, v, m, _ = gpu_solve(torch, B, I1, I2, 1, R, it, BOX)
+    margin = it * (R + 3 + 2) + 4
+    for (x0, y0) in ((0, 0), (W - 300, H - 260), (1900, 1500), (W - 300, 0)):
+        cw, ch = 300, 260
+        ref = oracle.solve(I1[y0:y0 + ch, x0:x0 + cw], I2[y0:y0 + ch, x0:x0 + cw], 1, R, it, BOX)
+        sl = (slice(margin, ch - margin), slice(margin, cw - margin))
+        gsl = (slice(y0 + margin, y0 + ch - margin), slice(x0 + margin, x0 + cw - margin))
+        sub = {k: ref[k][sl] for k in ("u", "v", "det", "valid")}
+        assert_parity(u[gsl], v[gsl], m[gsl], sub, ("crop", x0, y0))
+
+
+def test_errors_are_reported_not_thrown(B):
+    assert B.lib().of_create(64, 64, 3, 8, 1, 0) in (None, 0)      # 16x16 < 17
+    assert "coarsest" in B.last_error()
+    assert B.lib().of_create(64, 64, 1, 17, 1, 0) in (None, 0)
+    assert B.lib().of_create(64, 64, 1, 4, 0, 0) in (None, 0)
+    assert B.lib().of_create(64, 64, 1, 4, 1, 7) in (None, 0)
+    assert B.lib().of_compute(None, None, None, None, None, None) < 0
+    B.lib().of_destroy(None)

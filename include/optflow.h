@@ -100,10 +100,11 @@ int of_last_launch_count(of_handle h);
  *   its last iteration);  4..8: the five horizontally summed product planes left by the last
  *   products kernel (valid only for the level it ran on);  9: det = a*c - b^2 (level 0 only). */
 int of_get_debug_plane(of_handle h, int level, int which, float *out_dev, void *stream);
-/* Run ONE kernel of the iteration on the handle's internal state of `level`:
+/* Run ONE kernel of the iteration, `repeat` >= 1 times back to back, on the handle's internal state
+ * of `level` (for per-kernel timing and intermediate parity):
  *   which 0: warp + gradients + products + horizontal sum (K2);  1: vertical sum + solve + update (K3,
  *   in place on the internal field). */
-int of_run_step(of_handle h, int level, int which, void *stream);
+int of_run_step(of_handle h, int level, int which, int repeat, void *stream);
 
 /* Stand-alone single steps (rows a2, a10 of the scope table), dense device buffers. */
 int of_pyramid_down(const float *src, int width, int height, float *dst, void *stream);

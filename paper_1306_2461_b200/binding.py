@@ -34,7 +34,7 @@ SIGNATURES = {
     "of_level_size": (_i, [_vp, _i, _c.POINTER(_i), _c.POINTER(_i)]),
     "of_last_launch_count": (_i, [_vp]),
     "of_get_debug_plane": (_i, [_vp, _i, _i, _vp, _vp]),
-    "of_run_step": (_i, [_vp, _i, _i, _vp]),
+    "of_run_step": (_i, [_vp, _i, _i, _i, _vp]),
     "of_pyramid_down": (_i, [_vp, _i, _i, _vp, _vp]),
     "of_upsample_flow": (_i, [_vp, _vp, _i, _i, _vp, _vp, _i, _i, _vp]),
     "of_stream_open": (_i, [_vp, _i, _i, _i]),
@@ -165,8 +165,8 @@ class OpticalFlow:
         _check(lib().of_get_debug_plane(self._h, level, which, out.data_ptr(), _stream_ptr(stream)))
         return out
 
-    def run_step(self, level, which, stream=None):
-        _check(lib().of_run_step(self._h, level, which, _stream_ptr(stream)))
+    def run_step(self, level, which, repeat=1, stream=None):
+        _check(lib().of_run_step(self._h, level, which, repeat, _stream_ptr(stream)))
 
     # -- frame pipeline -----------------------------------------------------------------------
     def stream_open(self, dtype, mode=OF_STREAM_CONSECUTIVE, result_on_host=True):

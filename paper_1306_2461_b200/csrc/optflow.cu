@@ -230,7 +230,7 @@ int submit_job(of_context *c, const Job &j, cudaStream_t st)
     cudaError_t e3 = cudaGraphInstantiate(&exec, graph, 0);
     cudaGraphDestroy(graph);
     if (e3 != cudaSuccess) return fail(OF_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e3));
-    if (c->graphs.size() >= 8) {
+    if (c->graphs.size() >= 64) {
         size_t old = 0;
         for (size_t i = 1; i < c->graphs.size(); ++i)
             if (c->graphs[i].stamp < c->graphs[old].stamp) old = i;
@@ -454,12 +454,14 @@ int of_get_debug_plane(of_handle h, int level, int which, float *out_dev, void *
     return copy_plane_dense(src, L.pitch, L.W, L.H, out_dev, (cudaStream_t)stream);
 }
 
-int of_run_step(of_handle h, int level, int which, void *stream)
+int of_run_step(of_handle h, int level, int which, int repeat, void *stream)
 {
-    if (!h || level < 0 || level >= h->levels || which < 0 || which > 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    if (!h || level < 0 || level >= h->levels || which < 0 || which > 1 || repeat < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
     CU_TRY(cudaSetDevice(h->device));
-    if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], (cudaStream_t)stream);
-    else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, (cudaStream_t)stream);
+    for (int i = 0; i < repeat; ++i) {
+        if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], (cudaStream_t)stream);
+        else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, (cudaStream_t)stream);
+    }
     CU_TRY(cudaGetLastError());
     return OF_OK;
 }

@@ -203,10 +203,10 @@ def config2(width=1024, height=1024):
                     width, height, 2, 7, 6, WINDOW_BOX, tu, tv, {"input": "u8"})
 
 
-def config3(width=1280, height=1024):
+def config3(width=1280, height=1024, seed_offset=0):
     """BASELINE.json:9 -- 1280x1024 uint8, 0.025 ppp, backward-facing-step-like field (tanh shear,
     8 px max, -1 px recirculation), 3 levels, Gaussian window sigma 4 (R = 12), 10 iterations."""
-    rng = np.random.default_rng(SEED_BASE + 3)
+    rng = np.random.default_rng(SEED_BASE + 3 + 1000 * seed_offset)
     f1, f2, tu, tv = _pair_from_field(rng, width, height, 0.025, 1.2, 150.0, 255.0,
                                       field_backward_step(width, height))
     return FlowCase("config3", quantize(f1, np.uint8, 255), quantize(f2, np.uint8, 255),

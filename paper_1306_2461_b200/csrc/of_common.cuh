@@ -1,0 +1,13 @@
+// of_common.cuh -- small shared definitions of the sm_100a kernels (no arithmetic of the method).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define OFK_MAX_R 16
+
+struct WinWeights { float w[2 * OFK_MAX_R + 1]; };   // w[t + R], t = -R..R; passed by value (param bank)
+
+__device__ __forceinline__ int clampi(int i, int lo, int hi) { return max(lo, min(i, hi)); }
+
+// packed fp32 pair FMA with a scalar weight (FFMA2 on sm_100a: half the issue slots of two FFMA)
+__device__ __forceinline__ float2 fma2s(float w, float2 x, float2 acc) { return __ffma2_rn(x, make_float2(w, w), acc); }

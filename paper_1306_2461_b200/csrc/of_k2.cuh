@@ -1,0 +1,165 @@
+// of_k2.cuh -- K2: bilinear warp of I2 + central differences of I1 + It + five products + horizontal
+// window sum (rows a4-a7 of the scope table; BASELINE.json:5 "(2) Per-iteration warp+gradient+product
+// kernel"; readings D8-D12 of DESIGN.md).
+//
+// Warp-autonomous design for sm_100a: every WARP owns a tile of (8*nseg) x (2*nrp) outputs
+// (nseg*nrp <= 32) and a private slice of shared memory; there is no block-level barrier, so the
+// LSU-heavy product phase of one warp overlaps the FMA-heavy sum phase of the others on the same SM.
+//
+//   phase 1 (products): lane task = 2 columns x 2 rows.  All loads of I1/u/v are 8-byte vectors, I2
+//       is gathered with 4 scalar loads per pixel (L1/L2 hits: the field is smooth).  The products of
+//       a ROW PAIR are stored interleaved, {row y, row y+1} per column, so that phase 2 reads
+//       register pairs that feed the packed fp32 FMA (FFMA2) directly.
+//   phase 2 (horizontal sum): lane task = 8 adjacent outputs x 2 rows x 5 fields: (8+2RL)/2
+//       LDS.128 and 8*(2R+1) FFMA2 per field; the window weight is the scalar (broadcast) operand.
+//       Direct (2R+1)-tap sums: no running sums, no cancellation (H2), zero stays zero (D14 mask).
+//
+// Shared-memory layout per (field, row pair): column c at byte 8*c + 16*(c>>3) (16 B of padding per
+// 8 columns -> the LDS.128 of phase 2, 64 B apart between lanes, are bank-conflict free).
+#pragma once
+#include "of_common.cuh"
+
+#define K2_MAX_WARPS 16                            // warps per CTA (independent of each other); runtime blockDim
+
+template <int R> struct K2Geom {
+    static constexpr int RL = (R + 3) / 4 * 4;     // left/right halo rounded up: aligned vector loads
+    static constexpr int OFF = RL - R;             // first tap sits OFF columns into the halo
+    static constexpr int NIN = 8 + 2 * RL;         // input columns per phase-2 lane
+    __host__ __device__ static constexpr int pw(int nseg) { return 8 * nseg + 2 * RL; }
+    __host__ __device__ static constexpr int block_bytes(int nseg) { return pw(nseg) * 10; }
+    __host__ __device__ static constexpr int warp_bytes(int nseg, int nrp) { return 5 * nrp * block_bytes(nseg); }
+};
+
+struct K2Params {
+    const float *I1, *I2, *u, *v;
+    float *S;
+    size_t plane;
+    int W, H, pitch;
+    int nseg, nrp;                                 // lane layout of a warp tile
+    int tiles_y, ntiles;                           // tile t -> (tx = t / tiles_y, ty = t % tiles_y)
+    WinWeights ww;
+};
+
+// One pixel: bilinear sample of I2 at (x+u, y+v) (D8: integer part added to the integer index),
+// It = I2w - I1 - Ix*u - Iy*v (D10), five products.  gx, gy are already multiplied by the validity
+// mask (0 outside the image -> all five products are zero, D12).
+__device__ __forceinline__ void k2_pixel(const float *__restrict__ I2, int x, int y, int W, int H, int pitch,
+                                         float uu, float vv, float c, float gx, float gy,
+                                         float &xx, float &xy, float &yy, float &xt, float &yt)
+{
+    const float uc = fminf(fmaxf(uu, -16777216.f), 16777216.f);
+    const float vc = fminf(fmaxf(vv, -16777216.f), 16777216.f);
+    const float ax = uu - floorf(uu), ay = vv - floorf(vv);
+    const int X = x + __float2int_rd(uc), Y = y + __float2int_rd(vc);
+    const int xa = max(0, min(X, W - 1)), xb = max(0, min(X + 1, W - 1));
+    const int ra = max(0, min(Y, H - 1)) * pitch, rb = max(0, min(Y + 1, H - 1)) * pitch;
+    const float i00 = __ldg(I2 + ra + xa), i01 = __ldg(I2 + ra + xb);
+    const float i10 = __ldg(I2 + rb + xa), i11 = __ldg(I2 + rb + xb);
+    const float bx = 1.0f - ax, by = 1.0f - ay;
+    const float top = fmaf(ax, i01, bx * i00);
+    const float bot = fmaf(ax, i11, bx * i10);
+    const float I2w = fmaf(ay, bot, by * top);
+    const float It = fmaf(-gy, vv, fmaf(-gx, uu, I2w - c));
+    xx = gx * gx; xy = gx * gy; yy = gy * gy; xt = gx * It; yt = gy * It;
+}
+
+template <int R>
+__global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K2Params p)
+{
+    typedef K2Geom<R> G;
+    extern __shared__ float4 smem4[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nseg = p.nseg, nrp = p.nrp;
+    const int PW = G::pw(nseg), half = PW >> 1, BB = G::block_bytes(nseg);
+    char *const sm = reinterpret_cast<char *>(smem4) + warp * G::warp_bytes(nseg, nrp);
+    const int W = p.W, H = p.H, pitch = p.pitch;
+    const int ntasks = half * nrp;
+    const int TW = 8 * nseg, TH = 2 * nrp;
+    // phase-2 role of this lane
+    const int h_rp = lane / nseg, h_seg = lane - h_rp * nseg;
+
+    const int nw = blockDim.x >> 5;
+    for (int t = blockIdx.x * nw + warp; t < p.ntiles; t += gridDim.x * nw) {
+        const int tx = t / p.tiles_y, ty = t - tx * p.tiles_y;
+        const int x0 = tx * TW, y0 = ty * TH, xs = x0 - G::RL;
+
+        // ---------------- phase 1: products of (PW x TH) pixels -> shared memory
+#pragma unroll 1
+        for (int k = lane; k < ntasks; k += 32) {
+            int rp = 0, cp = k;
+            while (cp >= half) { cp -= half; ++rp; }
+            const int x = xs + 2 * cp, y = y0 + 2 * rp;
+            float4 o[5];
+#pragma unroll
+            for (int f = 0; f < 5; ++f) o[f] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (x >= 0 && x < W && y < H) {
+                const bool in1 = x + 1 < W, row1 = y + 1 < H;
+                const int ym = max(y - 1, 0), y1 = min(y + 1, H - 1), y2 = min(y + 2, H - 1);
+                const int xl = max(x - 1, 0), xr = min(x + 2, W - 1);
+                const int r0 = y * pitch, r1 = y1 * pitch;
+                const float2 cm = __ldg(reinterpret_cast<const float2 *>(p.I1 + ym * pitch + x));
+                const float2 c0 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r0 + x));
+                const float2 c1 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r1 + x));
+                const float2 c2 = __ldg(reinterpret_cast<const float2 *>(p.I1 + y2 * pitch + x));
+                const float2 u0 = __ldg(reinterpret_cast<const float2 *>(p.u + r0 + x));
+                const float2 u1 = __ldg(reinterpret_cast<const float2 *>(p.u + r1 + x));
+                const float2 v0 = __ldg(reinterpret_cast<const float2 *>(p.v + r0 + x));
+                const float2 v1 = __ldg(reinterpret_cast<const float2 *>(p.v + r1 + x));
+                const float l0 = __ldg(p.I1 + r0 + xl), q0 = __ldg(p.I1 + r0 + xr);
+                const float l1 = __ldg(p.I1 + r1 + xl), q1 = __ldg(p.I1 + r1 + xr);
+                const float m01 = in1 ? 0.5f : 0.f, m10 = row1 ? 0.5f : 0.f, m11 = (in1 && row1) ? 0.5f : 0.f;
+                // (x, y)
+                k2_pixel(p.I2, x, y, W, H, pitch, u0.x, v0.x, c0.x, 0.5f * ((in1 ? c0.y : c0.x) - l0), 0.5f * (c1.x - cm.x),
+                         o[0].x, o[1].x, o[2].x, o[3].x, o[4].x);
+                // (x, y+1)
+                k2_pixel(p.I2, x, y + 1, W, H, pitch, u1.x, v1.x, c1.x, m10 * ((in1 ? c1.y : c1.x) - l1), m10 * (c2.x - c0.x),
+                         o[0].y, o[1].y, o[2].y, o[3].y, o[4].y);
+                // (x+1, y)
+                k2_pixel(p.I2, x + 1, y, W, H, pitch, u0.y, v0.y, c0.y, m01 * (q0 - c0.x), m01 * (c1.y - cm.y),
+                         o[0].z, o[1].z, o[2].z, o[3].z, o[4].z);
+                // (x+1, y+1)
+                k2_pixel(p.I2, x + 1, y + 1, W, H, pitch, u1.y, v1.y, c1.y, m11 * (q1 - c1.x), m11 * (c2.y - c0.y),
+                         o[0].w, o[1].w, o[2].w, o[3].w, o[4].w);
+            }
+            char *d = sm + rp * BB + cp * 16 + (cp >> 2) * 16;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
+        }
+        __syncwarp();
+
+        // ---------------- phase 2: horizontal window sum, 8 outputs x 2 rows per lane
+        if (h_rp < nrp) {
+            const int gx = x0 + 8 * h_seg, gy = y0 + 2 * h_rp;
+            const char *src = sm + h_rp * BB + h_seg * 80;
+#pragma unroll 1
+            for (int f = 0; f < 5; ++f) {
+                float2 in[G::NIN];
+#pragma unroll
+                for (int k = 0; k < G::NIN / 2; ++k) {
+                    const float4 q = *reinterpret_cast<const float4 *>(src + f * nrp * BB + 16 * k + 16 * (k >> 2));
+                    in[2 * k] = make_float2(q.x, q.y);
+                    in[2 * k + 1] = make_float2(q.z, q.w);
+                }
+                float2 acc[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) acc[j] = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int tap = 0; tap <= 2 * R; ++tap)
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) acc[j] = fma2s(p.ww.w[tap], in[j + tap + G::OFF], acc[j]);
+                if (gx < pitch) {
+                    float *d0 = p.S + f * p.plane + (size_t)gy * pitch + gx;
+                    if (gy < H) {
+                        *reinterpret_cast<float4 *>(d0) = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);
+                        *reinterpret_cast<float4 *>(d0 + 4) = make_float4(acc[4].x, acc[5].x, acc[6].x, acc[7].x);
+                    }
+                    if (gy + 1 < H) {
+                        *reinterpret_cast<float4 *>(d0 + pitch) = make_float4(acc[0].y, acc[1].y, acc[2].y, acc[3].y);
+                        *reinterpret_cast<float4 *>(d0 + pitch + 4) = make_float4(acc[4].y, acc[5].y, acc[6].y, acc[7].y);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    }
+}

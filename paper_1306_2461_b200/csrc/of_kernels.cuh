@@ -4,21 +4,13 @@
 //   K0 convert_frames        a1   uint8/uint16/fp32 frame -> fp32 internal plane (exact, no scaling)
 //   K1 pyramid_down          a2   [1 4 6 4 1]/16 separable low-pass + 2x decimation, fused
 //   K4 upsample_flow         a10  u_l = 2*bilinear(u_{l+1}; x/2, y/2)
-//   K2 products_hsum         a4-a7 bilinear warp of I2, central differences of I1, It, five
-//                                 products, horizontal window sum -> five planes
-//   K3 vsum_solve            a8-a9 vertical window sum, damped 2x2 solve, clamp, in-place update
+//   K2 products_hsum         a4-a7 -> of_k2.cuh
+//   K3 vsum_solve            a8-a9 -> of_k3.cuh
 //
 // All internal planes of a level share one pitch (multiple of 32 floats, rows 128-byte aligned).
 // Shares no code with oracle/.
 #pragma once
-#include <cuda_runtime.h>
-#include <stdint.h>
-
-#define OFK_MAX_R 16
-
-struct WinWeights { float w[2 * OFK_MAX_R + 1]; };   // w[t + R], t = -R..R; passed by value (param bank)
-
-__device__ __forceinline__ int clampi(int i, int lo, int hi) { return max(lo, min(i, hi)); }
+#include "of_common.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // K0: frame conversion (row a1).  One thread per 4 pixels; src is dense (pitch == W), dst pitched.
@@ -126,188 +118,3 @@ __global__ void __launch_bounds__(256) k4_upsample_flow(const float *__restrict_
     v[(size_t)y * pitch + x] = 2.0f * ((1.0f - fy) * vt + fy * vb);
 }
 
-// ------------------------------------------------------------------------------------------------
-// The five products at one pixel (rows a4-a6).  D8: the integer part of the displacement is added
-// to the integer pixel index (x+u is never formed in fp32); D9: gradients of I1, clamped; D10:
-// It = I2w - I1 - Ix*u - Iy*v.
-// ------------------------------------------------------------------------------------------------
-struct Prod5 { float xx, xy, yy, xt, yt; };
-
-__device__ __forceinline__ Prod5 pixel_products(const float *__restrict__ I1, const float *__restrict__ I2,
-                                                const float *__restrict__ u, const float *__restrict__ v,
-                                                int x, int y, int W, int H, int pitch)
-{
-    const size_t row = (size_t)y * pitch;
-    const float uu = __ldg(u + row + x), vv = __ldg(v + row + x);
-    float fu = floorf(uu), fv = floorf(vv);
-    const float ax = uu - fu, ay = vv - fv;
-    fu = fminf(fmaxf(fu, -1.0e9f), 1.0e9f);
-    fv = fminf(fmaxf(fv, -1.0e9f), 1.0e9f);
-    const int X = x + (int)fu, Y = y + (int)fv;
-    const int xa = clampi(X, 0, W - 1), xb = clampi(X + 1, 0, W - 1);
-    const size_t ra = (size_t)clampi(Y, 0, H - 1) * pitch, rb = (size_t)clampi(Y + 1, 0, H - 1) * pitch;
-    const float top = (1.0f - ax) * __ldg(I2 + ra + xa) + ax * __ldg(I2 + ra + xb);
-    const float bot = (1.0f - ax) * __ldg(I2 + rb + xa) + ax * __ldg(I2 + rb + xb);
-    const float I2w = (1.0f - ay) * top + ay * bot;
-    const float c = __ldg(I1 + row + x);
-    const float Ix = 0.5f * (__ldg(I1 + row + min(x + 1, W - 1)) - __ldg(I1 + row + max(x - 1, 0)));
-    const float Iy = 0.5f * (__ldg(I1 + (size_t)min(y + 1, H - 1) * pitch + x) -
-                             __ldg(I1 + (size_t)max(y - 1, 0) * pitch + x));
-    const float It = I2w - c - Ix * uu - Iy * vv;
-    Prod5 p;
-    p.xx = Ix * Ix; p.xy = Ix * Iy; p.yy = Iy * Iy; p.xt = Ix * It; p.yt = Iy * It;
-    return p;
-}
-
-// ------------------------------------------------------------------------------------------------
-// K2: warp + gradients + products + horizontal window sum (rows a4-a7).
-// CTA = 128 x 16 outputs, 256 threads.  Phase 1: products on (128+2R) x 16 pixels -> shared memory
-// (zero outside the image: D12).  Phase 2: each thread sums 8 adjacent outputs of one row for each
-// field from registers (8+2R inputs -> 8(2R+1) FMAs).
-// ------------------------------------------------------------------------------------------------
-#define K2_TW 128
-#define K2_TH 16
-#define K2_SEG 8
-template <int R> struct K2Cfg {
-    static constexpr int PW = K2_TW + 2 * R;                       // product columns per row
-    static constexpr int NL = (K2_SEG + 2 * R + 3) / 4;            // float4 loads per thread per field
-    static constexpr int PITCH = K2_TW - K2_SEG + 4 * NL;          // smem row pitch (multiple of 4)
-    static constexpr size_t SMEM = sizeof(float) * 5 * K2_TH * PITCH;
-};
-
-template <int R>
-__global__ void __launch_bounds__(256) k2_products_hsum(const float *__restrict__ I1, const float *__restrict__ I2,
-                                                        const float *__restrict__ u, const float *__restrict__ v,
-                                                        float *__restrict__ S, size_t plane, int W, int H, int pitch,
-                                                        const WinWeights ww)
-{
-    typedef K2Cfg<R> C;
-    extern __shared__ float4 smem4[];
-    float *sm = reinterpret_cast<float *>(smem4);
-    const int x0 = blockIdx.x * K2_TW, y0 = blockIdx.y * K2_TH;
-
-    for (int i = threadIdx.x; i < C::PW * K2_TH; i += 256) {
-        const int r = i / C::PW, c = i - r * C::PW;
-        const int gx = x0 - R + c, gy = y0 + r;
-        Prod5 p = {0.f, 0.f, 0.f, 0.f, 0.f};
-        if (gx >= 0 && gx < W && gy < H) p = pixel_products(I1, I2, u, v, gx, gy, W, H, pitch);
-        float *d = sm + r * C::PITCH + c;
-        d[0 * K2_TH * C::PITCH] = p.xx;
-        d[1 * K2_TH * C::PITCH] = p.xy;
-        d[2 * K2_TH * C::PITCH] = p.yy;
-        d[3 * K2_TH * C::PITCH] = p.xt;
-        d[4 * K2_TH * C::PITCH] = p.yt;
-    }
-    __syncthreads();
-
-    const int r = threadIdx.x >> 4, seg = threadIdx.x & 15;
-    const int gy = y0 + r, gx = x0 + seg * K2_SEG;
-    if (gy >= H || gx >= pitch) return;
-#pragma unroll 1
-    for (int f = 0; f < 5; ++f) {
-        float in[4 * C::NL];
-        const float4 *src = reinterpret_cast<const float4 *>(sm + (f * K2_TH + r) * C::PITCH + seg * K2_SEG);
-#pragma unroll
-        for (int k = 0; k < C::NL; ++k) {
-            float4 t = src[k];
-            in[4 * k] = t.x; in[4 * k + 1] = t.y; in[4 * k + 2] = t.z; in[4 * k + 3] = t.w;
-        }
-        float acc[K2_SEG];
-#pragma unroll
-        for (int j = 0; j < K2_SEG; ++j) acc[j] = 0.f;
-#pragma unroll
-        for (int t = 0; t <= 2 * R; ++t)
-#pragma unroll
-            for (int j = 0; j < K2_SEG; ++j) acc[j] = fmaf(ww.w[t], in[j + t], acc[j]);
-        float4 *dst = reinterpret_cast<float4 *>(S + f * plane + (size_t)gy * pitch + gx);
-        dst[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-        dst[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// K3: vertical window sum + damped 2x2 solve + update (rows a8-a9).
-// CTA = 64 x 32 outputs, 256 threads.  Phase 1: (32+2R) rows x 64 columns of the five planes ->
-// shared memory (zero outside the image: D12).  Phase 2: each thread owns one column and 8 rows:
-// 8+2R inputs per field stream through registers into 8 accumulators; then the solve (D14, D15).
-// ------------------------------------------------------------------------------------------------
-#define K3_TW 64
-#define K3_TH 32
-#define K3_SEG 8
-template <int R> struct K3Cfg {
-    static constexpr int ROWS = K3_TH + 2 * R;
-    static constexpr size_t SMEM = sizeof(float) * 5 * ROWS * K3_TW;
-};
-
-struct SolveParams { float eps_half; float max_step; };
-
-template <int R>
-__global__ void __launch_bounds__(256) k3_vsum_solve(const float *__restrict__ S, size_t plane,
-                                                     const float *u_in, const float *v_in,   // may alias u_out, v_out
-                                                     float *u_out, float *v_out, int out_pitch,
-                                                     uint8_t *__restrict__ valid, float *__restrict__ det,
-                                                     int W, int H, int pitch, const WinWeights ww, const SolveParams sp)
-{
-    typedef K3Cfg<R> C;
-    extern __shared__ float4 smem4[];
-    float *sm = reinterpret_cast<float *>(smem4);
-    const int x0 = blockIdx.x * K3_TW, y0 = blockIdx.y * K3_TH;
-
-    // phase 1: 16 float4 per row
-    for (int i = threadIdx.x; i < 5 * C::ROWS * (K3_TW / 4); i += 256) {
-        const int c4 = i & 15, rr = i >> 4;
-        const int f = rr / C::ROWS, r = rr - f * C::ROWS;
-        const int gy = y0 - R + r, gx = x0 + 4 * c4;
-        float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (gy >= 0 && gy < H && gx < pitch)
-            t = __ldg(reinterpret_cast<const float4 *>(S + f * plane + (size_t)gy * pitch + gx));
-        reinterpret_cast<float4 *>(sm)[i] = t;
-    }
-    __syncthreads();
-
-    const int c = threadIdx.x & 63, g = threadIdx.x >> 6;
-    const int gx = x0 + c;
-    if (gx >= W) return;
-    float acc[5][K3_SEG];
-#pragma unroll
-    for (int f = 0; f < 5; ++f) {
-#pragma unroll
-        for (int j = 0; j < K3_SEG; ++j) acc[f][j] = 0.f;
-        const float *col = sm + (f * C::ROWS + g * K3_SEG) * K3_TW + c;
-#pragma unroll
-        for (int r = 0; r < K3_SEG + 2 * R; ++r) {
-            const float val = col[r * K3_TW];
-#pragma unroll
-            for (int j = 0; j < K3_SEG; ++j) {
-                const int t = r - j;
-                if (t >= 0 && t <= 2 * R) acc[f][j] = fmaf(ww.w[t], val, acc[f][j]);
-            }
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < K3_SEG; ++j) {
-        const int gy = y0 + g * K3_SEG + j;
-        if (gy >= H) break;
-        const size_t k = (size_t)gy * pitch + gx;
-        const float a = acc[0][j], b = acc[1][j], cc = acc[2][j], p = acc[3][j], q = acc[4][j];
-        const float uu = u_in[k], vv = v_in[k];
-        const float tr = a + cc;
-        float du = 0.f, dv = 0.f;
-        if (tr > 0.f) {
-            const float lam = sp.eps_half * tr;
-            const float A = a + lam, Cc = cc + lam;
-            const float D = A * Cc - b * b;
-            const float rp = -(p + a * uu + b * vv);
-            const float rq = -(q + b * uu + cc * vv);
-            du = (Cc * rp - b * rq) / D;
-            dv = (A * rq - b * rp) / D;
-            du = fminf(fmaxf(du, -sp.max_step), sp.max_step);
-            dv = fminf(fmaxf(dv, -sp.max_step), sp.max_step);
-        }
-        const size_t ko = (size_t)gy * out_pitch + gx;
-        u_out[ko] = uu + du;
-        v_out[ko] = vv + dv;
-        if (valid) valid[(size_t)gy * W + gx] = tr > 0.f ? 1 : 0;
-        if (det) det[k] = a * cc - b * b;
-    }
-}

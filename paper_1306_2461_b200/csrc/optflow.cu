@@ -5,8 +5,12 @@
 // reach the GPU returns an error.
 #include "../../include/optflow.h"
 #include "of_kernels.cuh"
+#include "of_k2.cuh"
+#include "of_k3.cuh"
 
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -39,6 +43,11 @@ int fail(int code, const char *fmt, ...)
     } while (0)
 
 struct Level { int W, H, pitch; };
+
+// Launch geometry of the two iteration kernels at one level (chosen once in of_create).
+struct K2Plan { int nseg, nrp, tiles_y, ntiles, grid, warps, smem; };
+struct K3Plan { int nrb, ntasks, grid, warps, smem; };
+constexpr int SMEM_MAX = 227 * 1024;
 
 // One enqueue of the whole path.  Also the key of the graph cache.
 struct Job {
@@ -85,10 +94,15 @@ struct of_context {
     float *det;
     uint8_t *valid;
     WinWeights ww;
+    int sms;
+    K2Plan k2[OF_MAX_LEVELS];
+    K3Plan k3[OF_MAX_LEVELS];
+    CUtensorMap tmS[OF_MAX_LEVELS];     // the five summed planes of a level as one (x, y, field) tensor
     bool use_graph;
     std::vector<GraphEntry> graphs;
     unsigned long long stamp;
     int last_launches;
+    std::string launch_err;            // first failing launch of the last enqueue ("" if none)
     std::vector<void *> allocs;
     Pipeline pipe;
 };
@@ -99,28 +113,120 @@ inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
 template <int R> int setup_attrs()
 {
-    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K2Cfg<R>::SMEM));
-    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K3Cfg<R>::SMEM));
+    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
+}
+
+// K2: warp tiles of (8*nseg) x (2*nrp) outputs, one CTA of `warps` independent warps per SM.  The
+// model below only ranks candidates: issue-bound time per SM vs the serial latency of one warp.
+template <int R> K2Plan plan_k2(int W, int H, int sms)
+{
+    typedef K2Geom<R> G;
+    K2Plan best = {};
+    double best_cost = 1e30;
+    int f_nseg = 0, f_nrp = 0, f_wps = 0;
+    if (const char *e = getenv("OF_K2_GEOM")) sscanf(e, "%d,%d,%d", &f_nseg, &f_nrp, &f_wps);
+    const int segs = (W + 7) / 8;
+    for (int nrp = 1; nrp <= 4; nrp *= 2) {
+        const int nsegmax = 32 / nrp, tx_min = (segs + nsegmax - 1) / nsegmax;
+        for (int tx = tx_min; tx <= tx_min + 3; ++tx) {
+            int nseg = (segs + tx - 1) / tx;
+            if (f_nseg) { if (nrp != f_nrp) continue; nseg = std::min(f_nseg, nsegmax); }
+            const int txr = (segs + nseg - 1) / nseg;
+            const int tasks = G::pw(nseg) / 2 * nrp, rounds = (tasks + 31) / 32;
+            const int ty = (H + 2 * nrp - 1) / (2 * nrp), ntiles = txr * ty;
+            const int wb = G::warp_bytes(nseg, nrp);
+            const int wmax = std::min(16, SMEM_MAX / wb);
+            for (int wps = 1; wps <= wmax; ++wps) {
+                if (f_wps && wps != f_wps) continue;
+                const int per = (ntiles + sms * wps - 1) / (sms * wps);
+                const double tile_instr = rounds * 250.0 + 1250.0;
+                const double lat = per * (rounds * 1500.0 + 2300.0);
+                const int conc = std::min(wps, (ntiles + sms - 1) / sms);
+                const double ipc = std::min(2.4, 0.35 * conc);
+                const double thr = (double)per * wps * tile_instr / ipc;
+                const double cost = std::max(lat, thr);
+                if (cost < best_cost) {
+                    best_cost = cost;
+                    const int w = std::max(1, std::min(wps, (ntiles + sms - 1) / sms));
+                    best = {nseg, nrp, ty, ntiles, std::min(sms, (ntiles + w - 1) / w), w, w * wb};
+                }
+            }
+            if (f_nseg) break;
+        }
+    }
+    return best;
+}
+
+// K3: tasks of 64 columns x 8 rows, equal contiguous share per CTA, one CTA per SM, NW tasks per step.
+template <int R> K3Plan plan_k3(int W, int H, int sms)
+{
+    K3Plan p = {};
+    p.nrb = (H + 7) / 8;
+    p.ntasks = ((W + 63) / 64) * p.nrb;
+    p.grid = std::min(sms, p.ntasks);
+    const int tpc = (p.ntasks + p.grid - 1) / p.grid;
+    int best = 1, best_cost = 1 << 30;
+    for (int nw = 1; nw <= K3_MAX_NW; ++nw) {
+        if (K3Geom<R>::smem_bytes(nw) > SMEM_MAX) break;
+        const int cost = (tpc + nw - 1) / nw * std::max(4, nw);
+        if (cost <= best_cost) { best_cost = cost; best = nw; }
+    }
+    if (const char *e = getenv("OF_K3_NW")) { int v = atoi(e); if (v >= 1 && v <= K3_MAX_NW && K3Geom<R>::smem_bytes(v) <= SMEM_MAX) best = v; }
+    p.warps = best;
+    p.smem = K3Geom<R>::smem_bytes(best);
+    return p;
+}
+
+template <int R> void plan_level(of_context *c, int l)
+{
+    c->k2[l] = plan_k2<R>(c->lv[l].W, c->lv[l].H, c->sms);
+    c->k3[l] = plan_k3<R>(c->lv[l].W, c->lv[l].H, c->sms);
 }
 
 template <int R>
 void launch_k2(const of_context *c, int l, const float *I1, const float *I2, cudaStream_t st)
 {
     const Level &L = c->lv[l];
-    dim3 grid((L.W + K2_TW - 1) / K2_TW, (L.H + K2_TH - 1) / K2_TH);
-    k2_products_hsum<R><<<grid, 256, K2Cfg<R>::SMEM, st>>>(I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, c->ww);
+    const K2Plan &P = c->k2[l];
+    K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, P.ntiles, c->ww};
+    k2_products_hsum<R><<<P.grid, 32 * P.warps, P.smem, st>>>(p);
 }
 
 template <int R>
 void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, cudaStream_t st)
 {
     const Level &L = c->lv[l];
-    dim3 grid((L.W + K3_TW - 1) / K3_TW, (L.H + K3_TH - 1) / K3_TH);
-    SolveParams sp = {0.5f * c->eps_rel, c->max_step};
-    k3_vsum_solve<R><<<grid, 256, K3Cfg<R>::SMEM, st>>>(c->S, c->plane, c->u[l], c->v[l], u_out, v_out, out_pitch,
-                                                        last ? c->valid : nullptr, last ? c->det : nullptr, L.W, L.H,
-                                                        L.pitch, c->ww, sp);
+    const K3Plan &P = c->k3[l];
+    K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
+                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}};
+    k3_vsum_solve<R><<<P.grid, 32 * P.warps, P.smem, st>>>(c->tmS[l], p);
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency:
+// the library must load on a machine without a driver, cf. tests/test_abi_cpu.py).
+int encode_tensor_maps(of_context *c)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CU_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return fail(OF_ERR_CUDA, "cuTensorMapEncodeTiled is not available in this driver");
+    for (int l = 0; l < c->levels; ++l) {
+        const Level &L = c->lv[l];
+        cuuint64_t dims[3] = {(cuuint64_t)L.pitch, (cuuint64_t)L.H, 5};
+        cuuint64_t strides[2] = {(cuuint64_t)L.pitch * sizeof(float), (cuuint64_t)c->plane * sizeof(float)};
+        cuuint32_t box[3] = {64, 8, 5};
+        cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = ((encode_fn)fn)(&c->tmS[l], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, c->S, dims, strides, box, estr,
+                                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(OF_ERR_CUDA, "cuTensorMapEncodeTiled(level %d) failed: CUresult %d", l, (int)r);
+    }
+    return OF_OK;
 }
 
 #define DISPATCH_R(R_, CALL)                                                                       \
@@ -171,30 +277,46 @@ void run_upsample(const of_context *c, int l, cudaStream_t st)   // level l+1 ->
     k4_upsample_flow<<<grid, 256, 0, st>>>(c->u[l + 1], c->v[l + 1], Cc.W, Cc.H, Cc.pitch, c->u[l], c->v[l], F.W, F.H, F.pitch);
 }
 
+void note_launch(of_context *c, const char *what, int level)
+{
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess && c->launch_err.empty()) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "%s (level %d): %s", what, level, cudaGetErrorString(e));
+        c->launch_err = buf;
+    }
+}
+
 // Enqueue the whole path of one Job (rows a1-a10).  Returns the number of kernels launched.
 int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
 {
     int n = 0;
+    c->launch_err.clear();
     if (j.cvtA >= 0) {
         const bool both = j.cvtB >= 0;
         run_convert(c, j.dtype, j.rawA, both ? j.rawB : nullptr, c->pyr[j.cvtA][0], both ? c->pyr[j.cvtB][0] : nullptr, st);
+        note_launch(c, "convert", 0);
         ++n;
         for (int l = 0; l + 1 < c->levels; ++l) {
             run_pyramid(c, l, c->pyr[j.cvtA][l], both ? c->pyr[j.cvtB][l] : nullptr, c->pyr[j.cvtA][l + 1],
                         both ? c->pyr[j.cvtB][l + 1] : nullptr, st);
+            note_launch(c, "pyramid", l);
             ++n;
         }
     }
     const int top = c->levels - 1;
     cudaMemsetAsync(c->u[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
     cudaMemsetAsync(c->v[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
+    note_launch(c, "memset", top);
     for (int l = top; l >= 0; --l) {
-        if (l < top) { run_upsample(c, l, st); ++n; }
+        if (l < top) { run_upsample(c, l, st); note_launch(c, "upsample", l); ++n; }
         for (int it = 0; it < c->iterations; ++it) {
             run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], st);
+            note_launch(c, "products+hsum", l);
             const bool last = (l == 0 && it == c->iterations - 1);
             if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, st);
             else run_k3(c, l, c->u[l], c->v[l], c->lv[l].pitch, false, st);
+            note_launch(c, "vsum+solve", l);
             n += 2;
         }
     }
@@ -206,7 +328,8 @@ int submit_job(of_context *c, const Job &j, cudaStream_t st)
     CU_TRY(cudaSetDevice(c->device));
     if (!c->use_graph || st == nullptr) {
         c->last_launches = enqueue_job(c, j, st);
-        CU_TRY(cudaGetLastError());
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail(OF_ERR_CUDA, "launch failed: %s; first failing launch: %s", cudaGetErrorString(e), c->launch_err.c_str());
         return OF_OK;
     }
     ++c->stamp;
@@ -224,7 +347,8 @@ int submit_job(of_context *c, const Job &j, cudaStream_t st)
     cudaError_t e2 = cudaStreamEndCapture(st, &graph);
     if (e1 != cudaSuccess || e2 != cudaSuccess || graph == nullptr) {
         if (graph) cudaGraphDestroy(graph);
-        return fail(OF_ERR_CUDA, "graph capture failed: %s / %s", cudaGetErrorString(e1), cudaGetErrorString(e2));
+        return fail(OF_ERR_CUDA, "graph capture failed: %s / %s; first failing launch: %s", cudaGetErrorString(e1), cudaGetErrorString(e2),
+                    c->launch_err.c_str());
     }
     cudaGraphExec_t exec = nullptr;
     cudaError_t e3 = cudaGraphInstantiate(&exec, graph, 0);
@@ -376,6 +500,16 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         if (cudaDeviceSynchronize() != cudaSuccess) rc = fail(OF_ERR_CUDA, "memset failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
     if (rc == OF_OK) { DISPATCH_R(window_radius, rc = setup_attrs<R>()); }
+    if (rc == OF_OK) {
+        c->sms = prop.multiProcessorCount;
+        for (int l = 0; l < levels; ++l) { DISPATCH_R(window_radius, plan_level<R>(c, l)); }
+        rc = encode_tensor_maps(c);
+        if (getenv("OF_DEBUG"))
+            for (int l = 0; l < levels; ++l)
+                fprintf(stderr, "[optflow] level %d %dx%d pitch %d | K2 nseg %d nrp %d tiles %d grid %d warps %d smem %d | K3 tasks %d grid %d warps %d smem %d\n",
+                        l, lv[l].W, lv[l].H, lv[l].pitch, c->k2[l].nseg, c->k2[l].nrp, c->k2[l].ntiles, c->k2[l].grid, c->k2[l].warps,
+                        c->k2[l].smem, c->k3[l].ntasks, c->k3[l].grid, c->k3[l].warps, c->k3[l].smem);
+    }
     if (rc != OF_OK) { std::string keep = g_err; of_destroy(c); g_err = keep; return nullptr; }
     return c;
 }

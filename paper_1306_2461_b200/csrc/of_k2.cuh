@@ -40,25 +40,62 @@ struct K2Params {
     WinWeights ww;
 };
 
-// One pixel: bilinear sample of I2 at (x+u, y+v) (D8: integer part added to the integer index),
-// It = I2w - I1 - Ix*u - Iy*v (D10), five products.  gx, gy are already multiplied by the validity
-// mask (0 outside the image -> all five products are zero, D12).
-__device__ __forceinline__ void k2_pixel(const float *__restrict__ I2, int x, int y, int W, int H, int pitch,
-                                         float uu, float vv, float c, float gx, float gy,
-                                         float &xx, float &xy, float &yy, float &xt, float &yt)
+// Inputs of one phase-1 task (2 columns x 2 rows): I1 rows y-1..y+2 at columns x, x+1, the left and
+// right neighbours of both rows, and the current field.  Loaded one round ahead (software prefetch).
+struct K2In {
+    float2 cm, c0, c1, c2, u0, u1, v0, v1;
+    float l0, q0, l1, q1;
+};
+
+__device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
 {
-    const float uc = fminf(fmaxf(uu, -16777216.f), 16777216.f);
-    const float vc = fminf(fmaxf(vv, -16777216.f), 16777216.f);
-    const float ax = uu - floorf(uu), ay = vv - floorf(vv);
-    const int X = x + __float2int_rd(uc), Y = y + __float2int_rd(vc);
-    const int xa = max(0, min(X, W - 1)), xb = max(0, min(X + 1, W - 1));
-    const int ra = max(0, min(Y, H - 1)) * pitch, rb = max(0, min(Y + 1, H - 1)) * pitch;
-    const float i00 = __ldg(I2 + ra + xa), i01 = __ldg(I2 + ra + xb);
-    const float i10 = __ldg(I2 + rb + xa), i11 = __ldg(I2 + rb + xb);
+    K2In in;
+    const int W = p.W, H = p.H, pitch = p.pitch;
+    const int ym = max(y - 1, 0), y1 = min(y + 1, H - 1), y2 = min(y + 2, H - 1);
+    const int xl = max(x - 1, 0), xr = min(x + 2, W - 1);
+    const int r0 = y * pitch, r1 = y1 * pitch;
+    in.cm = __ldg(reinterpret_cast<const float2 *>(p.I1 + ym * pitch + x));
+    in.c0 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r0 + x));
+    in.c1 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r1 + x));
+    in.c2 = __ldg(reinterpret_cast<const float2 *>(p.I1 + y2 * pitch + x));
+    in.u0 = __ldg(reinterpret_cast<const float2 *>(p.u + r0 + x));
+    in.u1 = __ldg(reinterpret_cast<const float2 *>(p.u + r1 + x));
+    in.v0 = __ldg(reinterpret_cast<const float2 *>(p.v + r0 + x));
+    in.v1 = __ldg(reinterpret_cast<const float2 *>(p.v + r1 + x));
+    in.l0 = __ldg(p.I1 + r0 + xl);
+    in.q0 = __ldg(p.I1 + r0 + xr);
+    in.l1 = __ldg(p.I1 + r1 + xl);
+    in.q1 = __ldg(p.I1 + r1 + xr);
+    return in;
+}
+
+// Bilinear sample of I2 at (x+u, y+v) (D8: the integer part of the displacement is added to the
+// integer pixel index; x+u is never formed in fp32).  Clamp-to-edge is applied as: clamp the cell
+// origin to [0, W-2] x [0, H-2] and force the fraction to 0 / 1 outside, which selects the same
+// pixels as clamping both taps (and is exact at the borders), with two row pointers + immediate
+// offsets instead of four separate addresses.
+__device__ __forceinline__ float k2_sample(const float *__restrict__ I2, int x, int y, int Wm2, int Hm2, int pitch, float uu, float vv)
+{
+    const float fu = floorf(uu), fv = floorf(vv);
+    float ax = uu - fu, ay = vv - fv;
+    const int X = x + (int)fminf(fmaxf(fu, -65536.f), 65536.f);
+    const int Y = y + (int)fminf(fmaxf(fv, -65536.f), 65536.f);
+    ax = X < 0 ? 0.f : (X > Wm2 ? 1.f : ax);
+    ay = Y < 0 ? 0.f : (Y > Hm2 ? 1.f : ay);
+    const float *p0 = I2 + (max(0, min(Y, Hm2)) * pitch + max(0, min(X, Wm2)));
+    const float *p1 = p0 + pitch;
+    const float i00 = __ldg(p0), i01 = __ldg(p0 + 1), i10 = __ldg(p1), i11 = __ldg(p1 + 1);
     const float bx = 1.0f - ax, by = 1.0f - ay;
     const float top = fmaf(ax, i01, bx * i00);
     const float bot = fmaf(ax, i11, bx * i10);
-    const float I2w = fmaf(ay, bot, by * top);
+    return fmaf(ay, bot, by * top);
+}
+
+// It = I2w - I1 - Ix*u - Iy*v (D10) and the five products.  gx, gy are already multiplied by the
+// validity mask (0 outside the image -> all five products are zero, D12).
+__device__ __forceinline__ void k2_products(float I2w, float uu, float vv, float c, float gx, float gy,
+                                            float &xx, float &xy, float &yy, float &xt, float &yt)
+{
     const float It = fmaf(-gy, vv, fmaf(-gx, uu, I2w - c));
     xx = gx * gx; xy = gx * gy; yy = gy * gy; xt = gx * It; yt = gy * It;
 }
@@ -84,46 +121,45 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
         const int x0 = tx * TW, y0 = ty * TH, xs = x0 - G::RL;
 
         // ---------------- phase 1: products of (PW x TH) pixels -> shared memory
+        // task k -> (row pair rp, column pair cp); inputs of round k+32 are in flight during round k
+        int rp = 0, cp = lane;
+        while (cp >= half) { cp -= half; ++rp; }
+        int x = xs + 2 * cp, y = y0 + 2 * rp;
+        bool ok = lane < ntasks && x >= 0 && x < W && y < H;
+        K2In cur = {};
+        if (ok) cur = k2_load(p, x, y);
 #pragma unroll 1
         for (int k = lane; k < ntasks; k += 32) {
-            int rp = 0, cp = k;
-            while (cp >= half) { cp -= half; ++rp; }
-            const int x = xs + 2 * cp, y = y0 + 2 * rp;
+            int nrp_ = rp, ncp = cp + 32;
+            while (ncp >= half) { ncp -= half; ++nrp_; }
+            const int nx = xs + 2 * ncp, ny = y0 + 2 * nrp_;
+            const bool nok = k + 32 < ntasks && nx >= 0 && nx < W && ny < H;
+            K2In nxt = {};
+            if (nok) nxt = k2_load(p, nx, ny);
+
             float4 o[5];
 #pragma unroll
             for (int f = 0; f < 5; ++f) o[f] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (x >= 0 && x < W && y < H) {
+            if (ok) {
                 const bool in1 = x + 1 < W, row1 = y + 1 < H;
-                const int ym = max(y - 1, 0), y1 = min(y + 1, H - 1), y2 = min(y + 2, H - 1);
-                const int xl = max(x - 1, 0), xr = min(x + 2, W - 1);
-                const int r0 = y * pitch, r1 = y1 * pitch;
-                const float2 cm = __ldg(reinterpret_cast<const float2 *>(p.I1 + ym * pitch + x));
-                const float2 c0 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r0 + x));
-                const float2 c1 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r1 + x));
-                const float2 c2 = __ldg(reinterpret_cast<const float2 *>(p.I1 + y2 * pitch + x));
-                const float2 u0 = __ldg(reinterpret_cast<const float2 *>(p.u + r0 + x));
-                const float2 u1 = __ldg(reinterpret_cast<const float2 *>(p.u + r1 + x));
-                const float2 v0 = __ldg(reinterpret_cast<const float2 *>(p.v + r0 + x));
-                const float2 v1 = __ldg(reinterpret_cast<const float2 *>(p.v + r1 + x));
-                const float l0 = __ldg(p.I1 + r0 + xl), q0 = __ldg(p.I1 + r0 + xr);
-                const float l1 = __ldg(p.I1 + r1 + xl), q1 = __ldg(p.I1 + r1 + xr);
                 const float m01 = in1 ? 0.5f : 0.f, m10 = row1 ? 0.5f : 0.f, m11 = (in1 && row1) ? 0.5f : 0.f;
-                // (x, y)
-                k2_pixel(p.I2, x, y, W, H, pitch, u0.x, v0.x, c0.x, 0.5f * ((in1 ? c0.y : c0.x) - l0), 0.5f * (c1.x - cm.x),
-                         o[0].x, o[1].x, o[2].x, o[3].x, o[4].x);
-                // (x, y+1)
-                k2_pixel(p.I2, x, y + 1, W, H, pitch, u1.x, v1.x, c1.x, m10 * ((in1 ? c1.y : c1.x) - l1), m10 * (c2.x - c0.x),
-                         o[0].y, o[1].y, o[2].y, o[3].y, o[4].y);
-                // (x+1, y)
-                k2_pixel(p.I2, x + 1, y, W, H, pitch, u0.y, v0.y, c0.y, m01 * (q0 - c0.x), m01 * (c1.y - cm.y),
-                         o[0].z, o[1].z, o[2].z, o[3].z, o[4].z);
-                // (x+1, y+1)
-                k2_pixel(p.I2, x + 1, y + 1, W, H, pitch, u1.y, v1.y, c1.y, m11 * (q1 - c1.x), m11 * (c2.y - c0.y),
-                         o[0].w, o[1].w, o[2].w, o[3].w, o[4].w);
+                const float s00 = k2_sample(p.I2, x, y, W - 2, H - 2, pitch, cur.u0.x, cur.v0.x);
+                const float s10 = k2_sample(p.I2, x, y + 1, W - 2, H - 2, pitch, cur.u1.x, cur.v1.x);
+                const float s01 = k2_sample(p.I2, x + 1, y, W - 2, H - 2, pitch, cur.u0.y, cur.v0.y);
+                const float s11 = k2_sample(p.I2, x + 1, y + 1, W - 2, H - 2, pitch, cur.u1.y, cur.v1.y);
+                k2_products(s00, cur.u0.x, cur.v0.x, cur.c0.x, 0.5f * ((in1 ? cur.c0.y : cur.c0.x) - cur.l0), 0.5f * (cur.c1.x - cur.cm.x),
+                            o[0].x, o[1].x, o[2].x, o[3].x, o[4].x);
+                k2_products(s10, cur.u1.x, cur.v1.x, cur.c1.x, m10 * ((in1 ? cur.c1.y : cur.c1.x) - cur.l1), m10 * (cur.c2.x - cur.c0.x),
+                            o[0].y, o[1].y, o[2].y, o[3].y, o[4].y);
+                k2_products(s01, cur.u0.y, cur.v0.y, cur.c0.y, m01 * (cur.q0 - cur.c0.x), m01 * (cur.c1.y - cur.cm.y),
+                            o[0].z, o[1].z, o[2].z, o[3].z, o[4].z);
+                k2_products(s11, cur.u1.y, cur.v1.y, cur.c1.y, m11 * (cur.q1 - cur.c1.x), m11 * (cur.c2.y - cur.c0.y),
+                            o[0].w, o[1].w, o[2].w, o[3].w, o[4].w);
             }
             char *d = sm + rp * BB + cp * 16 + (cp >> 2) * 16;
 #pragma unroll
             for (int f = 0; f < 5; ++f) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
+            cur = nxt; ok = nok; rp = nrp_; cp = ncp; x = nx; y = ny;
         }
         __syncwarp();
 

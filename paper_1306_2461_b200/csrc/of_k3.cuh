@@ -1,30 +1,36 @@
 // of_k3.cuh -- K3: vertical window sum + damped 2x2 solve + in-place (u,v) update (rows a8-a9 of the
 // scope table; BASELINE.json:5 "(3) Vertical-sum+solve kernel"; readings D11-D15 of DESIGN.md).
 //
-// Persistent, one CTA per SM, TMA-fed ring (sm_100a):
+// Persistent, warp-specialised, one CTA per SM (sm_100a):
 //   * the image is cut into 64-column strips x 8-row blocks = "tasks"; task order is strip-major and
 //     every CTA owns an equal, contiguous run of tasks (grid = number of SMs, no tail wave);
 //   * the five horizontally summed planes are ONE 3-D tensor (x, y, field); a chunk = box of
-//     64 x 8 x 5 floats (10 KB) fetched by a single cp.async.bulk.tensor into a shared-memory ring of
-//     2*NW + NC - 1 chunks; rows above/below the image are zero-filled by the TMA unit, which IS the
-//     zero extension of the window (D12) -- no border code;
-//   * step s: NW warps each take one task (8 rows x 64 columns; lane = 2 adjacent columns) while the
-//     chunks of step s+1 are in flight; one mbarrier per step parity, one __syncthreads per step;
-//   * per lane: (8+2R) LDS.64 per field feed 8*(2R+1) FFMA2 (packed fp32 pair FMA, scalar weight);
-//     then the damped 2x2 solve on the pair (D14), clamp (D15), update, validity byte.
-// Direct (2R+1)-tap sums, fixed order, no atomics: bit-reproducible (H8), no cancellation (H2).
+//     64 x 8 x 5 floats (10 KB) fetched by a single cp.async.bulk.tensor into a shared-memory ring;
+//     rows above/below the image are zero-filled by the TMA unit, which IS the zero extension of the
+//     window (D12) -- no border code;
+//   * one PRODUCER warp walks the CTA's chunks in order: waits for the ring slot to be released
+//     (empty mbarrier, NC arrivals = the NC tasks that read a chunk), arms the full mbarrier with
+//     expect_tx and issues the TMA;
+//   * up to 8 CONSUMER warps pull tasks from a shared-memory counter (balances the four SM
+//     sub-partitions), wait on the full barriers of their NC chunks, sum, release the chunks, solve.
+//     No __syncthreads after set-up.  Which warp runs a task does not change its arithmetic, so the
+//     result stays bit-reproducible (H8);
+//   * per lane (2 adjacent columns x 8 rows): (8+2R) LDS.64 per field feed 8*(2R+1) FFMA2 (packed
+//     fp32 pair FMA, scalar weight); then the damped 2x2 solve on the pair (D14), clamp (D15),
+//     update, validity byte.
+// Direct (2R+1)-tap sums, fixed order, no atomics on data: no cancellation (H2).
 #pragma once
 #include "of_common.cuh"
 #include <cuda.h>
 
 #define K3_CHUNK_BYTES (64 * 8 * 5 * 4)
-#define K3_MAX_NW 9
+#define K3_MAX_NW 8                                       // consumer warps (+1 producer warp)
+#define K3_RING 22                                        // chunks in the ring (220 KB)
 
 template <int R> struct K3Geom {
     static constexpr int NIN = 8 + 2 * R;                // input rows per task
     static constexpr int NC = (NIN + 7) / 8;             // chunks spanned by one task
-    __host__ __device__ static constexpr int ring(int nw) { return 2 * nw + NC - 1; }
-    __host__ __device__ static constexpr int smem_bytes(int nw) { return ring(nw) * K3_CHUNK_BYTES + 64; }
+    static constexpr int SMEM = K3_RING * K3_CHUNK_BYTES + 2 * K3_RING * 8 + 16;
 };
 
 struct SolveParams { float eps_half; float max_step; };
@@ -49,6 +55,10 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
@@ -95,17 +105,21 @@ __device__ __forceinline__ void k3_solve_pair(float2 a, float2 b, float2 c, floa
 }
 
 template <int R>
-__global__ void __launch_bounds__(32 * K3_MAX_NW, 1) k3_vsum_solve(const __grid_constant__ CUtensorMap tmS, const K3Params p)
+__global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const __grid_constant__ CUtensorMap tmS, const K3Params p)
 {
     typedef K3Geom<R> G;
+    constexpr int NC = G::NC;
     extern __shared__ __align__(1024) unsigned char k3_smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, NW = blockDim.x >> 5;
-    const int RING = G::ring(NW);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, NWC = (blockDim.x >> 5) - 1;
     const uint32_t ring0 = smem_u32(k3_smem);
-    const uint32_t bar0 = ring0 + RING * K3_CHUNK_BYTES;
+    const uint32_t full0 = ring0 + K3_RING * K3_CHUNK_BYTES, empty0 = full0 + 8 * K3_RING;
+    int *const counter = reinterpret_cast<int *>(k3_smem + K3_RING * K3_CHUNK_BYTES + 16 * K3_RING);
     if (threadIdx.x == 0) {
-        mbar_init(bar0, 1);
-        mbar_init(bar0 + 8, 1);
+        for (int j = 0; j < K3_RING; ++j) {
+            mbar_init(full0 + 8 * j, 1);
+            mbar_init(empty0 + 8 * j, NC);
+        }
+        *counter = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -113,93 +127,111 @@ __global__ void __launch_bounds__(32 * K3_MAX_NW, 1) k3_vsum_solve(const __grid_
     const int W = p.W, H = p.H, pitch = p.pitch, nrb = p.nrb;
     const int t_begin = (int)((long long)p.ntasks * blockIdx.x / gridDim.x);
     const int t_end = (int)((long long)p.ntasks * (blockIdx.x + 1) / gridDim.x);
-    uint32_t g = 0;                                                   // step counter: barrier g&1, parity (g>>1)&1
+    const int s_first = t_begin / nrb;
+    // Task i of this CTA (global task t_begin+i in strip s) reads ring chunks i + (s-s_first)*(NC-1) + k.
 
-    for (int t = t_begin; t < t_end;) {
-        const int strip = t / nrb, rb0 = t - strip * nrb;
-        const int ntask = min(nrb - rb0, t_end - t);
-        const int total = ntask + G::NC - 1;                           // chunks of this segment
-        const int x0 = strip * 64, yc0 = 8 * rb0 - R;                  // chunk c holds rows yc0+8c .. +7
-        const int nsteps = (ntask + NW - 1) / NW;
-        if (threadIdx.x == 0) {
-            const int n = min(NW + G::NC - 1, total);
-            const uint32_t bar = bar0 + 8 * (g & 1);
-            mbar_expect_tx(bar, n * K3_CHUNK_BYTES);
-            for (int c = 0; c < n; ++c) tma_load_3d(ring0 + (c % RING) * K3_CHUNK_BYTES, &tmS, x0, yc0 + 8 * c, 0, bar);
+    if (warp == NWC) {
+        // ===================== producer: one lane walks the chunks of every segment in order
+        if (lane == 0) {
+            for (int t = t_begin; t < t_end;) {
+                const int s = t / nrb, rb0 = t - s * nrb;
+                const int ntask = min(nrb - rb0, t_end - t);
+                const int total = ntask + NC - 1;
+                const int gbase = (t - t_begin) + (s - s_first) * (NC - 1);
+                const int x0 = 64 * s, yc0 = 8 * rb0 - R;               // chunk c holds rows yc0+8c .. +7
+                for (int c = 0; c < total; ++c) {
+                    const int gc = gbase + c, slot = gc % K3_RING, use = gc / K3_RING;
+                    if (use > 0) mbar_wait(empty0 + 8 * slot, (use - 1) & 1);
+                    const int readers = min(ntask - 1, c) - max(0, c - NC + 1) + 1;
+                    if (readers < NC) mbar_arrive(empty0 + 8 * slot, NC - readers);   // stand-ins for tasks that do not exist
+                    mbar_expect_tx(full0 + 8 * slot, K3_CHUNK_BYTES);
+                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, &tmS, x0, yc0 + 8 * c, 0, full0 + 8 * slot);
+                }
+                t += ntask;
+            }
         }
-        for (int s = 0; s < nsteps; ++s, ++g) {
-            if (threadIdx.x == 0 && s + 1 < nsteps) {
-                const int c_lo = NW * (s + 1) + G::NC - 1, c_hi = min(c_lo + NW, total);
-                const uint32_t bar = bar0 + 8 * ((g + 1) & 1);
-                mbar_expect_tx(bar, (c_hi - c_lo) * K3_CHUNK_BYTES);
-                for (int c = c_lo; c < c_hi; ++c) tma_load_3d(ring0 + (c % RING) * K3_CHUNK_BYTES, &tmS, x0, yc0 + 8 * c, 0, bar);
+        return;
+    }
+
+    // ========================= consumers
+    for (;;) {
+        int i = 0;
+        if (lane == 0) i = atomicAdd(counter, 1);
+        i = __shfl_sync(0xffffffffu, i, 0);
+        if (i >= t_end - t_begin) break;
+        const int gt = t_begin + i, s = gt / nrb, rb = gt - s * nrb;
+        const int gbase = i + (s - s_first) * (NC - 1);
+        const int gx = 64 * s + 2 * lane, gy0 = 8 * rb;
+        const bool active = gx < W;
+        // this lane's field values (issued before the waits: their latency hides behind them)
+        float2 uu[8], vv[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            uu[j] = make_float2(0.f, 0.f);
+            vv[j] = make_float2(0.f, 0.f);
+            if (active && gy0 + j < H) {
+                uu[j] = *reinterpret_cast<const float2 *>(p.u_in + (size_t)(gy0 + j) * pitch + gx);
+                vv[j] = *reinterpret_cast<const float2 *>(p.v_in + (size_t)(gy0 + j) * pitch + gx);
             }
-            const int task = s * NW + warp;
-            const int gx = x0 + 2 * lane, gy0 = 8 * (rb0 + task);
-            const bool active = task < ntask && gx < W;
-            // this lane's field values (issued before the wait: their latency hides behind it)
-            float2 uu[8], vv[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                uu[j] = make_float2(0.f, 0.f);
-                vv[j] = make_float2(0.f, 0.f);
-                if (active && gy0 + j < H) {
-                    uu[j] = *reinterpret_cast<const float2 *>(p.u_in + (size_t)(gy0 + j) * pitch + gx);
-                    vv[j] = *reinterpret_cast<const float2 *>(p.v_in + (size_t)(gy0 + j) * pitch + gx);
-                }
-            }
-            mbar_wait(bar0 + 8 * (g & 1), (g >> 1) & 1);
-            if (active) {
-                const unsigned char *cb[G::NC];
-#pragma unroll
-                for (int k = 0; k < G::NC; ++k) cb[k] = k3_smem + ((task + k) % RING) * K3_CHUNK_BYTES + lane * 8;
-                float2 acc[5][8];
-#pragma unroll
-                for (int f = 0; f < 5; ++f)
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) acc[f][j] = make_float2(0.f, 0.f);
-#pragma unroll
-                for (int r = 0; r < G::NIN; ++r) {
-#pragma unroll
-                    for (int f = 0; f < 5; ++f) {
-                        const float2 val = *reinterpret_cast<const float2 *>(cb[r >> 3] + f * 2048 + (r & 7) * 256);
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            if (r - j >= 0 && r - j <= 2 * R) acc[f][j] = fma2s(p.ww.w[r - j], val, acc[f][j]);
-                    }
-                }
-                const bool pair_ok = gx + 1 < W;
-                const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const int gy = gy0 + j;
-                    if (gy < H) {
-                        float2 du, dv, tr, det;
-                        k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, tr, det);
-                        const float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
-                        float *uo = p.u_out + (size_t)gy * p.out_pitch + gx, *vo = p.v_out + (size_t)gy * p.out_pitch + gx;
-                        if (vec_out) {
-                            *reinterpret_cast<float2 *>(uo) = un;
-                            *reinterpret_cast<float2 *>(vo) = vn;
-                        } else {
-                            uo[0] = un.x; vo[0] = vn.x;
-                            if (pair_ok) { uo[1] = un.y; vo[1] = vn.y; }
-                        }
-                        if (p.valid) {
-                            uint8_t *m = p.valid + (size_t)gy * W + gx;
-                            m[0] = tr.x > 0.f ? 1 : 0;
-                            if (pair_ok) m[1] = tr.y > 0.f ? 1 : 0;
-                        }
-                        if (p.det) {
-                            float *d = p.det + (size_t)gy * pitch + gx;
-                            d[0] = det.x;
-                            if (pair_ok) d[1] = det.y;
-                        }
-                    }
-                }
-            }
-            __syncthreads();
         }
-        t += ntask;
+        const unsigned char *cb[NC];
+        uint32_t eb[NC];
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            const int gc = gbase + k, slot = gc % K3_RING;
+            cb[k] = k3_smem + slot * K3_CHUNK_BYTES + lane * 8;
+            eb[k] = empty0 + 8 * slot;
+            mbar_wait(full0 + 8 * slot, (gc / K3_RING) & 1);
+        }
+        float2 acc[5][8];
+#pragma unroll
+        for (int f = 0; f < 5; ++f)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc[f][j] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int r = 0; r < G::NIN; ++r) {
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+                const float2 val = *reinterpret_cast<const float2 *>(cb[r >> 3] + f * 2048 + (r & 7) * 256);
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    if (r - j >= 0 && r - j <= 2 * R) acc[f][j] = fma2s(p.ww.w[r - j], val, acc[f][j]);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < NC; ++k) mbar_arrive(eb[k], 1);
+        }
+        if (!active) continue;
+        const bool pair_ok = gx + 1 < W;
+        const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int gy = gy0 + j;
+            if (gy < H) {
+                float2 du, dv, tr, det;
+                k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, tr, det);
+                const float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
+                float *uo = p.u_out + (size_t)gy * p.out_pitch + gx, *vo = p.v_out + (size_t)gy * p.out_pitch + gx;
+                if (vec_out) {
+                    *reinterpret_cast<float2 *>(uo) = un;
+                    *reinterpret_cast<float2 *>(vo) = vn;
+                } else {
+                    uo[0] = un.x; vo[0] = vn.x;
+                    if (pair_ok) { uo[1] = un.y; vo[1] = vn.y; }
+                }
+                if (p.valid) {
+                    uint8_t *m = p.valid + (size_t)gy * W + gx;
+                    m[0] = tr.x > 0.f ? 1 : 0;
+                    if (pair_ok) m[1] = tr.y > 0.f ? 1 : 0;
+                }
+                if (p.det) {
+                    float *d = p.det + (size_t)gy * pitch + gx;
+                    d[0] = det.x;
+                    if (pair_ok) d[1] = det.y;
+                }
+            }
+        }
     }
 }

@@ -167,15 +167,9 @@ template <int R> K3Plan plan_k3(int W, int H, int sms)
     p.ntasks = ((W + 63) / 64) * p.nrb;
     p.grid = std::min(sms, p.ntasks);
     const int tpc = (p.ntasks + p.grid - 1) / p.grid;
-    int best = 1, best_cost = 1 << 30;
-    for (int nw = 1; nw <= K3_MAX_NW; ++nw) {
-        if (K3Geom<R>::smem_bytes(nw) > SMEM_MAX) break;
-        const int cost = (tpc + nw - 1) / nw * std::max(4, nw);
-        if (cost <= best_cost) { best_cost = cost; best = nw; }
-    }
-    if (const char *e = getenv("OF_K3_NW")) { int v = atoi(e); if (v >= 1 && v <= K3_MAX_NW && K3Geom<R>::smem_bytes(v) <= SMEM_MAX) best = v; }
-    p.warps = best;
-    p.smem = K3Geom<R>::smem_bytes(best);
+    p.warps = std::min(K3_MAX_NW, tpc);                         // consumer warps; one producer warp is added at launch
+    if (const char *e = getenv("OF_K3_NW")) { int v = atoi(e); if (v >= 1 && v <= K3_MAX_NW) p.warps = v; }
+    p.smem = K3Geom<R>::SMEM;
     return p;
 }
 
@@ -201,7 +195,7 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     const K3Plan &P = c->k3[l];
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
                   L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}};
-    k3_vsum_solve<R><<<P.grid, 32 * P.warps, P.smem, st>>>(c->tmS[l], p);
+    k3_vsum_solve<R><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency:

@@ -38,6 +38,7 @@ struct K2Params {
     int nseg, nrp;                                 // lane layout of a warp tile
     int tiles_y, ntiles;                           // tile t -> (tx = t / tiles_y, ty = t % tiles_y)
     WinWeights ww;
+    int dbg;                                       // profiling switches (0 in production): 1 = no product phase, 2 = no sum phase
 };
 
 // Inputs of one phase-1 task (2 columns x 2 rows): I1 rows y-1..y+2 at columns x, x+1, the left and
@@ -129,7 +130,7 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
         K2In cur = {};
         if (ok) cur = k2_load(p, x, y);
 #pragma unroll 1
-        for (int k = lane; k < ntasks; k += 32) {
+        for (int k = lane; k < ntasks && !(p.dbg & 1); k += 32) {
             int nrp_ = rp, ncp = cp + 32;
             while (ncp >= half) { ncp -= half; ++nrp_; }
             const int nx = xs + 2 * ncp, ny = y0 + 2 * nrp_;
@@ -164,7 +165,7 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
         __syncwarp();
 
         // ---------------- phase 2: horizontal window sum, 8 outputs x 2 rows per lane
-        if (h_rp < nrp) {
+        if (h_rp < nrp && !(p.dbg & 2)) {
             const int gx = x0 + 8 * h_seg, gy = y0 + 2 * h_rp;
             const char *src = sm + h_rp * BB + h_seg * 80;
 #pragma unroll 1

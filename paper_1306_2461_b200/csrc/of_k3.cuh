@@ -24,7 +24,7 @@
 #include <cuda.h>
 
 #define K3_CHUNK_BYTES (64 * 8 * 5 * 4)
-#define K3_MAX_NW 8                                       // consumer warps (+1 producer warp)
+#define K3_MAX_NW 11                                      // consumer warps (+1 producer warp)
 #define K3_RING 22                                        // chunks in the ring (220 KB)
 
 template <int R> struct K3Geom {
@@ -44,6 +44,7 @@ struct K3Params {
     int nrb, ntasks;                 // row blocks per strip; ntasks = nstrips * nrb
     WinWeights ww;
     SolveParams sp;
+    int dbg;                         // profiling switches (0 in production): 1 = no TMA/no waits, 2 = no window sum, 4 = no solve
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -132,7 +133,7 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
 
     if (warp == NWC) {
         // ===================== producer: one lane walks the chunks of every segment in order
-        if (lane == 0) {
+        if (lane == 0 && !(p.dbg & 1)) {
             for (int t = t_begin; t < t_end;) {
                 const int s = t / nrb, rb0 = t - s * nrb;
                 const int ntask = min(nrb - rb0, t_end - t);
@@ -163,17 +164,6 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
         const int gbase = i + (s - s_first) * (NC - 1);
         const int gx = 64 * s + 2 * lane, gy0 = 8 * rb;
         const bool active = gx < W;
-        // this lane's field values (issued before the waits: their latency hides behind them)
-        float2 uu[8], vv[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            uu[j] = make_float2(0.f, 0.f);
-            vv[j] = make_float2(0.f, 0.f);
-            if (active && gy0 + j < H) {
-                uu[j] = *reinterpret_cast<const float2 *>(p.u_in + (size_t)(gy0 + j) * pitch + gx);
-                vv[j] = *reinterpret_cast<const float2 *>(p.v_in + (size_t)(gy0 + j) * pitch + gx);
-            }
-        }
         const unsigned char *cb[NC];
         uint32_t eb[NC];
 #pragma unroll
@@ -181,13 +171,14 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
             const int gc = gbase + k, slot = gc % K3_RING;
             cb[k] = k3_smem + slot * K3_CHUNK_BYTES + lane * 8;
             eb[k] = empty0 + 8 * slot;
-            mbar_wait(full0 + 8 * slot, (gc / K3_RING) & 1);
+            if (!(p.dbg & 1)) mbar_wait(full0 + 8 * slot, (gc / K3_RING) & 1);
         }
         float2 acc[5][8];
 #pragma unroll
         for (int f = 0; f < 5; ++f)
 #pragma unroll
             for (int j = 0; j < 8; ++j) acc[f][j] = make_float2(0.f, 0.f);
+        if (!(p.dbg & 2))
 #pragma unroll
         for (int r = 0; r < G::NIN; ++r) {
 #pragma unroll
@@ -199,37 +190,52 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
             }
         }
         __syncwarp();
-        if (lane == 0) {
+        if (lane == 0 && !(p.dbg & 1)) {
 #pragma unroll
             for (int k = 0; k < NC; ++k) mbar_arrive(eb[k], 1);
         }
-        if (!active) continue;
+        if (!active || (p.dbg & 4)) continue;
+        // ---- solve + update for 8 rows x 2 columns (field values are loaded here: TLP hides them)
+        const int nrows = min(8, H - gy0);
         const bool pair_ok = gx + 1 < W;
         const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
+        const float *ui = p.u_in + (size_t)gy0 * pitch + gx, *vi = p.v_in + (size_t)gy0 * pitch + gx;
+        float2 uu[8], vv[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            const int gy = gy0 + j;
-            if (gy < H) {
-                float2 du, dv, tr, det;
-                k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, tr, det);
-                const float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
-                float *uo = p.u_out + (size_t)gy * p.out_pitch + gx, *vo = p.v_out + (size_t)gy * p.out_pitch + gx;
+            uu[j] = make_float2(0.f, 0.f);
+            vv[j] = make_float2(0.f, 0.f);
+            if (j < nrows) {
+                uu[j] = *reinterpret_cast<const float2 *>(ui + j * pitch);
+                vv[j] = *reinterpret_cast<const float2 *>(vi + j * pitch);
+            }
+        }
+        float *uo = p.u_out + (size_t)gy0 * p.out_pitch + gx, *vo = p.v_out + (size_t)gy0 * p.out_pitch + gx;
+        float2 trs[8], dets[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            float2 du, dv;
+            k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, trs[j], dets[j]);
+            const float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
+            if (j < nrows) {
                 if (vec_out) {
-                    *reinterpret_cast<float2 *>(uo) = un;
-                    *reinterpret_cast<float2 *>(vo) = vn;
+                    *reinterpret_cast<float2 *>(uo + j * p.out_pitch) = un;
+                    *reinterpret_cast<float2 *>(vo + j * p.out_pitch) = vn;
                 } else {
-                    uo[0] = un.x; vo[0] = vn.x;
-                    if (pair_ok) { uo[1] = un.y; vo[1] = vn.y; }
+                    uo[j * p.out_pitch] = un.x; vo[j * p.out_pitch] = vn.x;
+                    if (pair_ok) { uo[j * p.out_pitch + 1] = un.y; vo[j * p.out_pitch + 1] = vn.y; }
                 }
-                if (p.valid) {
-                    uint8_t *m = p.valid + (size_t)gy * W + gx;
-                    m[0] = tr.x > 0.f ? 1 : 0;
-                    if (pair_ok) m[1] = tr.y > 0.f ? 1 : 0;
-                }
-                if (p.det) {
-                    float *d = p.det + (size_t)gy * pitch + gx;
-                    d[0] = det.x;
-                    if (pair_ok) d[1] = det.y;
+            }
+        }
+        if (p.valid) {                                   // last iteration of level 0 only
+            uint8_t *m = p.valid + (size_t)gy0 * W + gx;
+            float *d = p.det + (size_t)gy0 * pitch + gx;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                if (j < nrows) {
+                    m[j * W] = trs[j].x > 0.f ? 1 : 0;
+                    d[j * pitch] = dets[j].x;
+                    if (pair_ok) { m[j * W + 1] = trs[j].y > 0.f ? 1 : 0; d[j * pitch + 1] = dets[j].y; }
                 }
             }
         }

@@ -94,7 +94,7 @@ struct of_context {
     float *det;
     uint8_t *valid;
     WinWeights ww;
-    int sms;
+    int sms, dbg;
     K2Plan k2[OF_MAX_LEVELS];
     K3Plan k3[OF_MAX_LEVELS];
     CUtensorMap tmS[OF_MAX_LEVELS];     // the five summed planes of a level as one (x, y, field) tensor
@@ -184,7 +184,7 @@ void launch_k2(const of_context *c, int l, const float *I1, const float *I2, cud
 {
     const Level &L = c->lv[l];
     const K2Plan &P = c->k2[l];
-    K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, P.ntiles, c->ww};
+    K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, P.ntiles, c->ww, c->dbg};
     k2_products_hsum<R><<<P.grid, 32 * P.warps, P.smem, st>>>(p);
 }
 
@@ -194,7 +194,7 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     const Level &L = c->lv[l];
     const K3Plan &P = c->k3[l];
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
-                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}};
+                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, c->dbg};
     k3_vsum_solve<R><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
@@ -496,6 +496,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     if (rc == OF_OK) { DISPATCH_R(window_radius, rc = setup_attrs<R>()); }
     if (rc == OF_OK) {
         c->sms = prop.multiProcessorCount;
+        c->dbg = getenv("OF_KERNEL_DEBUG") ? atoi(getenv("OF_KERNEL_DEBUG")) : 0;
         for (int l = 0; l < levels; ++l) { DISPATCH_R(window_radius, plan_level<R>(c, l)); }
         rc = encode_tensor_maps(c);
         if (getenv("OF_DEBUG"))

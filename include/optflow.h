@@ -37,6 +37,7 @@ enum of_stream_mode { OF_STREAM_CONSECUTIVE = 0, OF_STREAM_PAIRS = 1 };
 
 #define OF_MAX_LEVELS 12
 #define OF_MAX_WINDOW_RADIUS 16
+#define OF_TIMELINE_MAX 4096
 
 /* ---------------------------------------------------------------------------------------------
  * The three calls named by the north_star (BASELINE.json:5).
@@ -84,6 +85,12 @@ int of_set_conditioning(of_handle h, float eps_rel, float max_step_px);
  * the caller's pointers change. */
 int of_set_graph(of_handle h, int enable);
 
+/* Run the whole solve of a pair (all levels, all iterations, flow hand-down) as ONE persistent
+ * cooperative kernel whose CTAs alternate the two iteration kernels' passes across a grid barrier
+ * (default on: a kernel boundary costs more than a coarse-level pass).  With 0, every pass is its own
+ * launch.  Both give bit-identical results. */
+int of_set_persistent(of_handle h, int enable);
+
 /* Validity bytes (1 = tr(G) > 0, D14) of the last iteration at level 0 of the last solve: copies
  * H x W bytes into the device buffer mask_dev, on `stream`. */
 int of_get_validity(of_handle h, uint8_t *mask_dev, void *stream);
@@ -91,7 +98,9 @@ int of_get_validity(of_handle h, uint8_t *mask_dev, void *stream);
 /* Size of pyramid level `level`. */
 int of_level_size(of_handle h, int level, int *width, int *height);
 
-/* Number of kernel launches (graph kernel nodes included) enqueued by the last of_compute* call. */
+/* Number of kernel launches (graph kernel nodes included) enqueued by the last of_compute* call:
+ * persistent mode 1 (convert) + levels-1 (pyramid) + 1 (solve); otherwise + levels-1 hand-downs and
+ * 2*levels*iterations iteration kernels instead of the solve. */
 int of_last_launch_count(of_handle h);
 
 /* Test / profiling hooks.  State is that left by the last of_compute* on this handle.
@@ -105,6 +114,16 @@ int of_get_debug_plane(of_handle h, int level, int which, float *out_dev, void *
  *   which 0: warp + gradients + products + horizontal sum (K2);  1: vertical sum + solve + update (K3,
  *   in place on the internal field). */
 int of_run_step(of_handle h, int level, int which, int repeat, void *stream);
+
+/* Timeline of the persistent solve kernel (profiling hook; the in-kernel analogue of a launch list).
+ * While the hook is on, thread 0 of every CTA stores its SM cycle counter, relative to the CTA's start,
+ * at every phase boundary (after a CTA-wide barrier; %globaltimer is refreshed too coarsely): start; per level coarse-to-fine { hand-down end, grid barrier end } (not for the
+ * coarsest); per iteration { K2 pass end, grid barrier end, K3 pass end, grid barrier end }.
+ * Copies the stamps of the last profiled solve to out_host (HOST pointer, may be NULL): those of CTA
+ * `cta`, or for cta < 0 the maximum over CTAs (when the last CTA reached each boundary).  Synchronises
+ * the device.  Then switches the hook on/off for the following solves.  Returns the number of entries
+ * written (0 if the hook was off), or a negative status. */
+int of_solve_timeline(of_handle h, int enable, int cta, unsigned long long *out_host, int max_entries);
 
 /* Stand-alone single steps (rows a2, a10 of the scope table), dense device buffers. */
 int of_pyramid_down(const float *src, int width, int height, float *dst, void *stream);

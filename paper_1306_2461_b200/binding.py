@@ -30,6 +30,8 @@ SIGNATURES = {
     "of_last_error": (_c.c_char_p, []),
     "of_set_conditioning": (_i, [_vp, _c.c_float, _c.c_float]),
     "of_set_graph": (_i, [_vp, _i]),
+    "of_set_persistent": (_i, [_vp, _i]),
+    "of_solve_timeline": (_i, [_vp, _i, _i, _vp, _i]),
     "of_get_validity": (_i, [_vp, _vp, _vp]),
     "of_level_size": (_i, [_vp, _i, _c.POINTER(_i), _c.POINTER(_i)]),
     "of_last_launch_count": (_i, [_vp]),
@@ -143,6 +145,19 @@ class OpticalFlow:
 
     def set_graph(self, enable: bool):
         _check(lib().of_set_graph(self._h, 1 if enable else 0))
+
+    def set_persistent(self, enable: bool):
+        _check(lib().of_set_persistent(self._h, 1 if enable else 0))
+
+    def solve_timeline(self, enable=True, cta=-1):
+        """Stamps [ns] of the last profiled solve (NumPy uint64, empty if the hook was off) of CTA
+        `cta`, or the maximum over CTAs for cta < 0; then switches the hook on/off."""
+        import numpy as np
+        buf = np.zeros(4096, dtype=np.uint64)
+        n = lib().of_solve_timeline(self._h, 1 if enable else 0, cta, buf.ctypes.data, buf.size)
+        if n < 0:
+            _check(n)
+        return buf[:n]
 
     def validity(self, stream=None):
         torch = self._torch

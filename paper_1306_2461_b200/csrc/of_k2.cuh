@@ -19,7 +19,7 @@
 #pragma once
 #include "of_common.cuh"
 
-#define K2_MAX_WARPS 16                            // warps per CTA (independent of each other); runtime blockDim
+#define K2_MAX_WARPS 12                            // warps per CTA (independent of each other); runtime blockDim
 
 template <int R> struct K2Geom {
     static constexpr int RL = (R + 3) / 4 * 4;     // left/right halo rounded up: aligned vector loads
@@ -43,6 +43,8 @@ struct K2Params {
 
 // Inputs of one phase-1 task (2 columns x 2 rows): I1 rows y-1..y+2 at columns x, x+1, the left and
 // right neighbours of both rows, and the current field.  Loaded one round ahead (software prefetch).
+// u, v are read through L2 only (ld.global.cg): the persistent solve kernel rewrites them between phases,
+// so the non-coherent L1 path must not be used for them; I1 / I2 are read-only for a whole solve.
 struct K2In {
     float2 cm, c0, c1, c2, u0, u1, v0, v1;
     float l0, q0, l1, q1;
@@ -52,21 +54,24 @@ __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
 {
     K2In in;
     const int W = p.W, H = p.H, pitch = p.pitch;
-    const int ym = max(y - 1, 0), y1 = min(y + 1, H - 1), y2 = min(y + 2, H - 1);
-    const int xl = max(x - 1, 0), xr = min(x + 2, W - 1);
-    const int r0 = y * pitch, r1 = y1 * pitch;
-    in.cm = __ldg(reinterpret_cast<const float2 *>(p.I1 + ym * pitch + x));
-    in.c0 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r0 + x));
-    in.c1 = __ldg(reinterpret_cast<const float2 *>(p.I1 + r1 + x));
-    in.c2 = __ldg(reinterpret_cast<const float2 *>(p.I1 + y2 * pitch + x));
-    in.u0 = __ldg(reinterpret_cast<const float2 *>(p.u + r0 + x));
-    in.u1 = __ldg(reinterpret_cast<const float2 *>(p.u + r1 + x));
-    in.v0 = __ldg(reinterpret_cast<const float2 *>(p.v + r0 + x));
-    in.v1 = __ldg(reinterpret_cast<const float2 *>(p.v + r1 + x));
-    in.l0 = __ldg(p.I1 + r0 + xl);
-    in.q0 = __ldg(p.I1 + r0 + xr);
-    in.l1 = __ldg(p.I1 + r1 + xl);
-    in.q1 = __ldg(p.I1 + r1 + xr);
+    const int i0 = y * pitch + x;                                  // one index, rows by +-pitch
+    const int dm = y > 0 ? -pitch : 0, d1 = y + 1 < H ? pitch : 0, d2 = (y + 2 < H ? pitch : 0) + d1;
+    const float *c = p.I1 + i0, *c1p = c + d1;
+    in.cm = __ldg(reinterpret_cast<const float2 *>(c + dm));
+    in.c0 = __ldg(reinterpret_cast<const float2 *>(c));
+    in.c1 = __ldg(reinterpret_cast<const float2 *>(c1p));
+    in.c2 = __ldg(reinterpret_cast<const float2 *>(c + d2));
+    const float *pu = p.u + i0, *pv = p.v + i0;
+    in.u0 = __ldcg(reinterpret_cast<const float2 *>(pu));
+    in.u1 = __ldcg(reinterpret_cast<const float2 *>(pu + d1));
+    in.v0 = __ldcg(reinterpret_cast<const float2 *>(pv));
+    in.v1 = __ldcg(reinterpret_cast<const float2 *>(pv + d1));
+    // left / right neighbours with clamp-to-edge: x-1 -> x at the left border, x+2 -> W-1 at the right
+    const int ol = x > 0 ? -1 : 0, orr = x + 2 < W ? 2 : (x + 1 < W ? 1 : 0);
+    in.l0 = __ldg(c + ol);
+    in.q0 = __ldg(c + orr);
+    in.l1 = __ldg(c1p + ol);
+    in.q1 = __ldg(c1p + orr);
     return in;
 }
 
@@ -74,22 +79,42 @@ __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
 // integer pixel index; x+u is never formed in fp32).  Clamp-to-edge is applied as: clamp the cell
 // origin to [0, W-2] x [0, H-2] and force the fraction to 0 / 1 outside, which selects the same
 // pixels as clamping both taps (and is exact at the borders), with two row pointers + immediate
-// offsets instead of four separate addresses.
-__device__ __forceinline__ float k2_sample(const float *__restrict__ I2, int x, int y, int Wm2, int Hm2, int pitch, float uu, float vv)
+// offsets instead of four separate addresses.  Split in two so that a lane can issue the gathers
+// of all its pixels before it consumes the first one.
+struct K2Tap { float i00, i01, i10, i11, ax, ay; };
+
+__device__ __forceinline__ K2Tap k2_gather(const float *__restrict__ I2, int x, int y, int Wm2, int Hm2, int pitch, float uu, float vv)
 {
+    K2Tap t;
     const float fu = floorf(uu), fv = floorf(vv);
-    float ax = uu - fu, ay = vv - fv;
+    t.ax = uu - fu;
+    t.ay = vv - fv;
     const int X = x + (int)fminf(fmaxf(fu, -65536.f), 65536.f);
     const int Y = y + (int)fminf(fmaxf(fv, -65536.f), 65536.f);
-    ax = X < 0 ? 0.f : (X > Wm2 ? 1.f : ax);
-    ay = Y < 0 ? 0.f : (Y > Hm2 ? 1.f : ay);
+    t.ax = X < 0 ? 0.f : (X > Wm2 ? 1.f : t.ax);
+    t.ay = Y < 0 ? 0.f : (Y > Hm2 ? 1.f : t.ay);
     const float *p0 = I2 + (max(0, min(Y, Hm2)) * pitch + max(0, min(X, Wm2)));
     const float *p1 = p0 + pitch;
-    const float i00 = __ldg(p0), i01 = __ldg(p0 + 1), i10 = __ldg(p1), i11 = __ldg(p1 + 1);
-    const float bx = 1.0f - ax, by = 1.0f - ay;
-    const float top = fmaf(ax, i01, bx * i00);
-    const float bot = fmaf(ax, i11, bx * i10);
-    return fmaf(ay, bot, by * top);
+    t.i00 = __ldg(p0); t.i01 = __ldg(p0 + 1); t.i10 = __ldg(p1); t.i11 = __ldg(p1 + 1);
+    return t;
+}
+
+__device__ __forceinline__ float k2_lerp(const K2Tap &t)
+{
+    const float bx = 1.0f - t.ax, by = 1.0f - t.ay;
+    const float top = fmaf(t.ax, t.i01, bx * t.i00);
+    const float bot = fmaf(t.ax, t.i11, bx * t.i10);
+    return fmaf(t.ay, bot, by * top);
+}
+
+// The four pixels of one phase-1 task: gathers first (k2_task_gather), products later (k2_task_products).
+__device__ __forceinline__ void k2_task_gather(const K2Params &p, const K2In &in, int x, int y, K2Tap (&t)[4])
+{
+    const int Wm2 = p.W - 2, Hm2 = p.H - 2;
+    t[0] = k2_gather(p.I2, x, y, Wm2, Hm2, p.pitch, in.u0.x, in.v0.x);
+    t[1] = k2_gather(p.I2, x, y + 1, Wm2, Hm2, p.pitch, in.u1.x, in.v1.x);
+    t[2] = k2_gather(p.I2, x + 1, y, Wm2, Hm2, p.pitch, in.u0.y, in.v0.y);
+    t[3] = k2_gather(p.I2, x + 1, y + 1, Wm2, Hm2, p.pitch, in.u1.y, in.v1.y);
 }
 
 // It = I2w - I1 - Ix*u - Iy*v (D10) and the five products.  gx, gy are already multiplied by the
@@ -101,75 +126,79 @@ __device__ __forceinline__ void k2_products(float I2w, float uu, float vv, float
     xx = gx * gx; xy = gx * gy; yy = gy * gy; xt = gx * It; yt = gy * It;
 }
 
+__device__ __forceinline__ void k2_task_products(const K2Params &p, const K2In &cur, int x, int y, const K2Tap (&t)[4], float4 (&o)[5])
+{
+    const bool in1 = x + 1 < p.W, row1 = y + 1 < p.H;
+    const float m01 = in1 ? 0.5f : 0.f, m10 = row1 ? 0.5f : 0.f, m11 = (in1 && row1) ? 0.5f : 0.f;
+    k2_products(k2_lerp(t[0]), cur.u0.x, cur.v0.x, cur.c0.x, 0.5f * ((in1 ? cur.c0.y : cur.c0.x) - cur.l0), 0.5f * (cur.c1.x - cur.cm.x),
+                o[0].x, o[1].x, o[2].x, o[3].x, o[4].x);
+    k2_products(k2_lerp(t[1]), cur.u1.x, cur.v1.x, cur.c1.x, m10 * ((in1 ? cur.c1.y : cur.c1.x) - cur.l1), m10 * (cur.c2.x - cur.c0.x),
+                o[0].y, o[1].y, o[2].y, o[3].y, o[4].y);
+    k2_products(k2_lerp(t[2]), cur.u0.y, cur.v0.y, cur.c0.y, m01 * (cur.q0 - cur.c0.x), m01 * (cur.c1.y - cur.cm.y),
+                o[0].z, o[1].z, o[2].z, o[3].z, o[4].z);
+    k2_products(k2_lerp(t[3]), cur.u1.y, cur.v1.y, cur.c1.y, m11 * (cur.q1 - cur.c1.x), m11 * (cur.c2.y - cur.c0.y),
+                o[0].w, o[1].w, o[2].w, o[3].w, o[4].w);
+}
+
+// One K2 pass over a level by CTA `cta` of `ncta`: the CTA owns an equal, contiguous range of warp
+// tiles and its warps pull tiles from `tile_counter` (shared memory, 0 on entry, CTA-synchronised), so
+// fast warps take more tiles.  Which warp computes a tile does not change its arithmetic.  `smem_cta`
+// is the CTA's dynamic shared memory, of which this warp uses slice `warp`.  Called by the stand-alone
+// kernel below and by the persistent solve kernel (of_solve.cuh).
 template <int R>
-__global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K2Params p)
+__device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_cta, int *tile_counter, int warp, int lane, int cta, int ncta)
 {
     typedef K2Geom<R> G;
-    extern __shared__ float4 smem4[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nseg = p.nseg, nrp = p.nrp;
     const int PW = G::pw(nseg), half = PW >> 1, BB = G::block_bytes(nseg);
-    char *const sm = reinterpret_cast<char *>(smem4) + warp * G::warp_bytes(nseg, nrp);
+    char *const sm = reinterpret_cast<char *>(smem_cta) + warp * G::warp_bytes(nseg, nrp);
     const int W = p.W, H = p.H, pitch = p.pitch;
     const int ntasks = half * nrp;
     const int TW = 8 * nseg, TH = 2 * nrp;
-    // phase-2 role of this lane
-    const int h_rp = lane / nseg, h_seg = lane - h_rp * nseg;
+    // phase-2 role of this lane: (field group, row pair, segment).  Small tiles (5*nseg*nrp <= 32) give
+    // every field its own lanes, which shortens the serial chain of a coarse-level pass five-fold.
+    const int nf_par = (5 * nseg * nrp <= 32) ? 5 : 1;
+    const int h_seg = lane % nseg, h_rp = (lane / nseg) % nrp, h_f0 = lane / (nseg * nrp);
 
-    const int nw = blockDim.x >> 5;
-    for (int t = blockIdx.x * nw + warp; t < p.ntiles; t += gridDim.x * nw) {
+    const int t_begin = (int)((long long)p.ntiles * cta / ncta), t_end = (int)((long long)p.ntiles * (cta + 1) / ncta);
+    for (;;) {
+        int t = 0;
+        if (lane == 0) t = atomicAdd(tile_counter, 1);
+        t = __shfl_sync(0xffffffffu, t, 0) + t_begin;
+        if (t >= t_end) break;
         const int tx = t / p.tiles_y, ty = t - tx * p.tiles_y;
         const int x0 = tx * TW, y0 = ty * TH, xs = x0 - G::RL;
 
         // ---------------- phase 1: products of (PW x TH) pixels -> shared memory
-        // task k -> (row pair rp, column pair cp); inputs of round k+32 are in flight during round k
-        int rp = 0, cp = lane;
-        while (cp >= half) { cp -= half; ++rp; }
-        int x = xs + 2 * cp, y = y0 + 2 * rp;
-        bool ok = lane < ntasks && x >= 0 && x < W && y < H;
-        K2In cur = {};
-        if (ok) cur = k2_load(p, x, y);
+        // task k -> (row pair rp, column pair cp): input loads, then the 16 gathers of its four pixels,
+        // then the arithmetic (other warps of the SM cover the two memory latencies)
 #pragma unroll 1
         for (int k = lane; k < ntasks && !(p.dbg & 1); k += 32) {
-            int nrp_ = rp, ncp = cp + 32;
-            while (ncp >= half) { ncp -= half; ++nrp_; }
-            const int nx = xs + 2 * ncp, ny = y0 + 2 * nrp_;
-            const bool nok = k + 32 < ntasks && nx >= 0 && nx < W && ny < H;
-            K2In nxt = {};
-            if (nok) nxt = k2_load(p, nx, ny);
-
+            int rp = 0, cp = k;
+            while (cp >= half) { cp -= half; ++rp; }
+            const int x = xs + 2 * cp, y = y0 + 2 * rp;
             float4 o[5];
+            if (x >= 0 && x < W && y < H) {
+                const K2In in = k2_load(p, x, y);
+                K2Tap t[4];
+                k2_task_gather(p, in, x, y, t);
+                k2_task_products(p, in, x, y, t, o);
+            } else {
 #pragma unroll
-            for (int f = 0; f < 5; ++f) o[f] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (ok) {
-                const bool in1 = x + 1 < W, row1 = y + 1 < H;
-                const float m01 = in1 ? 0.5f : 0.f, m10 = row1 ? 0.5f : 0.f, m11 = (in1 && row1) ? 0.5f : 0.f;
-                const float s00 = k2_sample(p.I2, x, y, W - 2, H - 2, pitch, cur.u0.x, cur.v0.x);
-                const float s10 = k2_sample(p.I2, x, y + 1, W - 2, H - 2, pitch, cur.u1.x, cur.v1.x);
-                const float s01 = k2_sample(p.I2, x + 1, y, W - 2, H - 2, pitch, cur.u0.y, cur.v0.y);
-                const float s11 = k2_sample(p.I2, x + 1, y + 1, W - 2, H - 2, pitch, cur.u1.y, cur.v1.y);
-                k2_products(s00, cur.u0.x, cur.v0.x, cur.c0.x, 0.5f * ((in1 ? cur.c0.y : cur.c0.x) - cur.l0), 0.5f * (cur.c1.x - cur.cm.x),
-                            o[0].x, o[1].x, o[2].x, o[3].x, o[4].x);
-                k2_products(s10, cur.u1.x, cur.v1.x, cur.c1.x, m10 * ((in1 ? cur.c1.y : cur.c1.x) - cur.l1), m10 * (cur.c2.x - cur.c0.x),
-                            o[0].y, o[1].y, o[2].y, o[3].y, o[4].y);
-                k2_products(s01, cur.u0.y, cur.v0.y, cur.c0.y, m01 * (cur.q0 - cur.c0.x), m01 * (cur.c1.y - cur.cm.y),
-                            o[0].z, o[1].z, o[2].z, o[3].z, o[4].z);
-                k2_products(s11, cur.u1.y, cur.v1.y, cur.c1.y, m11 * (cur.q1 - cur.c1.x), m11 * (cur.c2.y - cur.c0.y),
-                            o[0].w, o[1].w, o[2].w, o[3].w, o[4].w);
+                for (int f = 0; f < 5; ++f) o[f] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
             char *d = sm + rp * BB + cp * 16 + (cp >> 2) * 16;
 #pragma unroll
             for (int f = 0; f < 5; ++f) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
-            cur = nxt; ok = nok; rp = nrp_; cp = ncp; x = nx; y = ny;
         }
         __syncwarp();
 
         // ---------------- phase 2: horizontal window sum, 8 outputs x 2 rows per lane
-        if (h_rp < nrp && !(p.dbg & 2)) {
+        if (h_f0 < nf_par && !(p.dbg & 2)) {
             const int gx = x0 + 8 * h_seg, gy = y0 + 2 * h_rp;
             const char *src = sm + h_rp * BB + h_seg * 80;
 #pragma unroll 1
-            for (int f = 0; f < 5; ++f) {
+            for (int f = h_f0; f < 5; f += nf_par) {
                 float2 in[G::NIN];
 #pragma unroll
                 for (int k = 0; k < G::NIN / 2; ++k) {
@@ -199,4 +228,15 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
         }
         __syncwarp();
     }
+}
+
+template <int R>
+__global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K2Params p)
+{
+    extern __shared__ float4 smem4[];                          // warp slices, then 16 bytes for the tile counter
+    int *tile_counter = reinterpret_cast<int *>(reinterpret_cast<unsigned char *>(smem4) +
+                                                (blockDim.x >> 5) * K2Geom<R>::warp_bytes(p.nseg, p.nrp));
+    if (threadIdx.x == 0) *tile_counter = 0;
+    __syncthreads();
+    k2_phase<R>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, blockIdx.x, gridDim.x);
 }

@@ -105,31 +105,55 @@ __device__ __forceinline__ void k3_solve_pair(float2 a, float2 b, float2 c, floa
     dv.y = tr.y > 0.f ? fminf(fmaxf(dv.y, -ms), ms) : 0.f;
 }
 
+// Shared-memory carve-up of the K3 ring: chunks | full barriers | empty barriers | task counter.
+struct K3Smem {
+    unsigned char *base;
+    uint32_t ring0, full0, empty0;
+    int *counter;
+    __device__ __forceinline__ explicit K3Smem(unsigned char *b)
+        : base(b), ring0(smem_u32(b)), full0(ring0 + K3_RING * K3_CHUNK_BYTES), empty0(full0 + 8 * K3_RING),
+          counter(reinterpret_cast<int *>(b + K3_RING * K3_CHUNK_BYTES + 16 * K3_RING)) {}
+};
+
+// Thread 0 of the CTA, once per kernel, followed by __syncthreads.
+template <int R> __device__ __forceinline__ void k3_init_barriers(const K3Smem &sm)
+{
+    for (int j = 0; j < K3_RING; ++j) {
+        mbar_init(sm.full0 + 8 * j, 1);
+        mbar_init(sm.empty0 + 8 * j, K3Geom<R>::NC);
+    }
+    sm.counter[0] = 0;
+    sm.counter[1] = 0;                     // tile counter of the K2 pass in the persistent kernel
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+// Number of ring chunks CTA `cta` of `ncta` consumes in one K3 pass (uniform; advances the chunk base).
+template <int R> __device__ __forceinline__ int k3_cta_chunks(const K3Params &p, int cta, int ncta)
+{
+    const int t_begin = (int)((long long)p.ntasks * cta / ncta), t_end = (int)((long long)p.ntasks * (cta + 1) / ncta);
+    if (t_end <= t_begin) return 0;
+    return (t_end - t_begin) + ((t_end - 1) / p.nrb - t_begin / p.nrb + 1) * (K3Geom<R>::NC - 1);
+}
+
+// One K3 pass over a level by CTA `cta` of `ncta`.  Warp `nwc` (the last one) is the producer, warps
+// 0..nwc-1 consume.  `gc0` = number of ring chunks this CTA has consumed in earlier passes of the same
+// kernel (keeps slot / parity bookkeeping continuous); *sm.counter must be 0 on entry (CTA-synchronised).
+// All reads of u, v go through L2 (ld.global.cg): see of_k2.cuh.
 template <int R>
-__global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const __grid_constant__ CUtensorMap tmS, const K3Params p)
+__device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params &p, const K3Smem &sm, int warp, int lane, int nwc,
+                                         int cta, int ncta, uint32_t gc0)
 {
     typedef K3Geom<R> G;
     constexpr int NC = G::NC;
-    extern __shared__ __align__(1024) unsigned char k3_smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, NWC = (blockDim.x >> 5) - 1;
-    const uint32_t ring0 = smem_u32(k3_smem);
-    const uint32_t full0 = ring0 + K3_RING * K3_CHUNK_BYTES, empty0 = full0 + 8 * K3_RING;
-    int *const counter = reinterpret_cast<int *>(k3_smem + K3_RING * K3_CHUNK_BYTES + 16 * K3_RING);
-    if (threadIdx.x == 0) {
-        for (int j = 0; j < K3_RING; ++j) {
-            mbar_init(full0 + 8 * j, 1);
-            mbar_init(empty0 + 8 * j, NC);
-        }
-        *counter = 0;
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-
+    unsigned char *const k3_smem = sm.base;
+    const uint32_t ring0 = sm.ring0, full0 = sm.full0, empty0 = sm.empty0;
+    int *const counter = sm.counter;
+    const int NWC = nwc;
     const int W = p.W, H = p.H, pitch = p.pitch, nrb = p.nrb;
-    const int t_begin = (int)((long long)p.ntasks * blockIdx.x / gridDim.x);
-    const int t_end = (int)((long long)p.ntasks * (blockIdx.x + 1) / gridDim.x);
+    const int t_begin = (int)((long long)p.ntasks * cta / ncta);
+    const int t_end = (int)((long long)p.ntasks * (cta + 1) / ncta);
     const int s_first = t_begin / nrb;
-    // Task i of this CTA (global task t_begin+i in strip s) reads ring chunks i + (s-s_first)*(NC-1) + k.
+    // Task i of this CTA (global task t_begin+i in strip s) reads ring chunks gc0 + i + (s-s_first)*(NC-1) + k.
 
     if (warp == NWC) {
         // ===================== producer: one lane walks the chunks of every segment in order
@@ -138,7 +162,7 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
                 const int s = t / nrb, rb0 = t - s * nrb;
                 const int ntask = min(nrb - rb0, t_end - t);
                 const int total = ntask + NC - 1;
-                const int gbase = (t - t_begin) + (s - s_first) * (NC - 1);
+                const int gbase = (int)gc0 + (t - t_begin) + (s - s_first) * (NC - 1);
                 const int x0 = 64 * s, yc0 = 8 * rb0 - R;               // chunk c holds rows yc0+8c .. +7
                 for (int c = 0; c < total; ++c) {
                     const int gc = gbase + c, slot = gc % K3_RING, use = gc / K3_RING;
@@ -146,7 +170,7 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
                     const int readers = min(ntask - 1, c) - max(0, c - NC + 1) + 1;
                     if (readers < NC) mbar_arrive(empty0 + 8 * slot, NC - readers);   // stand-ins for tasks that do not exist
                     mbar_expect_tx(full0 + 8 * slot, K3_CHUNK_BYTES);
-                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, &tmS, x0, yc0 + 8 * c, 0, full0 + 8 * slot);
+                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + 8 * c, 0, full0 + 8 * slot);
                 }
                 t += ntask;
             }
@@ -161,7 +185,7 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
         i = __shfl_sync(0xffffffffu, i, 0);
         if (i >= t_end - t_begin) break;
         const int gt = t_begin + i, s = gt / nrb, rb = gt - s * nrb;
-        const int gbase = i + (s - s_first) * (NC - 1);
+        const int gbase = (int)gc0 + i + (s - s_first) * (NC - 1);
         const int gx = 64 * s + 2 * lane, gy0 = 8 * rb;
         const bool active = gx < W;
         const unsigned char *cb[NC];
@@ -206,8 +230,8 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
             uu[j] = make_float2(0.f, 0.f);
             vv[j] = make_float2(0.f, 0.f);
             if (j < nrows) {
-                uu[j] = *reinterpret_cast<const float2 *>(ui + j * pitch);
-                vv[j] = *reinterpret_cast<const float2 *>(vi + j * pitch);
+                uu[j] = __ldcg(reinterpret_cast<const float2 *>(ui + j * pitch));
+                vv[j] = __ldcg(reinterpret_cast<const float2 *>(vi + j * pitch));
             }
         }
         float *uo = p.u_out + (size_t)gy0 * p.out_pitch + gx, *vo = p.v_out + (size_t)gy0 * p.out_pitch + gx;
@@ -240,4 +264,14 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
             }
         }
     }
+}
+
+template <int R>
+__global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const __grid_constant__ CUtensorMap tmS, const K3Params p)
+{
+    extern __shared__ __align__(1024) unsigned char k3_smem_[];
+    const K3Smem sm(k3_smem_);
+    if (threadIdx.x == 0) k3_init_barriers<R>(sm);
+    __syncthreads();
+    k3_phase<R>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, blockIdx.x, gridDim.x, 0u);
 }

@@ -1,0 +1,166 @@
+// of_solve.cuh -- the persistent solve kernel: every level, every iteration of one frame pair in ONE
+// cooperative launch (rows a3-a10 of the scope table).
+//
+// Why: at 1280x1024 an iteration kernel runs 10-15 us and at the coarse levels 1-3 us, while a
+// kernel boundary costs 2-4 us on B200 (measured: an empty K2/K3 launch, back to back in a stream,
+// takes 4.1 us; profiles/r1_launch_overhead.md).  With ~65 launches per pair the boundaries were half
+// of the time.  Here one CTA per SM stays resident and the K2 pass (of_k2.cuh), the K3 pass
+// (of_k3.cuh) and the flow hand-down alternate, separated by a grid-wide barrier (one L2 atomic +
+// one acquire spin, < 1 us).  The decomposition of the method is unchanged: K2 still writes the five
+// horizontally summed planes, K3 still reads them back (through TMA) -- 72 B per pixel-iteration.
+//
+// Memory-model notes
+//   * u, v are rewritten by the K3 pass and read by the next K2 pass on other SMs: both sides use
+//     L2-only accesses (ld.global.cg) and the barrier carries __threadfence + acquire/release.
+//   * the five planes are written with ordinary stores and read by the TMA unit (async proxy): the
+//     producer lane issues fence.proxy.async after the barrier and before its first TMA.
+//   * shared memory is a union of the K2 warp slices and the K3 ring: fence.proxy.async.shared::cta
+//     after the K2 pass orders its generic-proxy stores before the TMA writes of the K3 pass.
+#pragma once
+#include "of_k2.cuh"
+#include "of_k3.cuh"
+
+#define SOLVE_TIMELINE_MAX 4096
+#define SOLVE_WARPS 12                       // 11 K3 consumers + 1 producer; all 12 work in the K2 pass
+
+struct LevelDesc {
+    const float *pyr[2];                     // pyramid slots (I1 / I2 chosen per job)
+    float *u, *v;
+    int W, H, pitch;
+    int k2_nseg, k2_nrp, k2_tiles_y, k2_ntiles;
+    int k3_nrb, k3_ntasks;
+};
+
+struct SolveArgs {
+    const LevelDesc *lv;                     // device array [levels]
+    const CUtensorMap *tm;                   // device array [levels], 64-byte aligned
+    unsigned *gbar;                          // {arrival count, generation}, zero-initialised once
+    float *S;
+    size_t plane;
+    float *u_out, *v_out;                    // dense level-0 result
+    uint8_t *valid;
+    float *det;
+    int levels, iterations, s1, s2, out_pitch, dbg;
+    unsigned long long *prof;                // optional timelines [ncta][SOLVE_TIMELINE_MAX] (SM clock at every phase boundary) or NULL
+    WinWeights ww;
+    SolveParams sp;
+};
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
+{
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Grid barrier k (k = 0, 1, ... within one launch) on a counter that is 0 at launch: every CTA adds 1
+// with release semantics and spins (acquire) until the counter reaches (k+1)*ncta.  One L2 atomic and
+// one or two L2 polls; no generation word, no reset between barriers.  grid_barrier_exit() returns the
+// counter to 0 when the last CTA leaves the kernel, so a captured graph can replay the launch.
+__device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned ncta, unsigned &k)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned target = (k + 1) * ncta;
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+        while (ld_acquire_u32(bar) < target) { }
+    }
+    ++k;
+    __syncthreads();
+}
+
+__device__ __forceinline__ void grid_barrier_exit(unsigned *bar, unsigned ncta)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned old = atomicInc(bar + 1, ncta - 1);      // wraps to 0 with the last CTA
+        if (old == ncta - 1) atomicExch(bar, 0u);                // every CTA has passed the last barrier
+    }
+}
+
+__device__ __forceinline__ void prof_stamp(const SolveArgs &a, int &idx)
+{
+    if (a.prof != nullptr) __syncthreads();                      // stamp when the whole CTA is done, not just warp 0
+    if (a.prof != nullptr && threadIdx.x == 0) {
+        // SM cycle counter: %globaltimer is refreshed too coarsely (several us) to time a pass
+        a.prof[(size_t)blockIdx.x * SOLVE_TIMELINE_MAX + idx] = (unsigned long long)clock64();
+    }
+    ++idx;
+}
+
+// Flow hand-down (row a10, D6): u_l = 2*bilinear(u_{l+1}; x/2, y/2), grid-stride over the fine level.
+__device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDesc &C, int gtid, int nthreads)
+{
+    const int W = F.W, H = F.H, Wc = C.W, Hc = C.H, cp = C.pitch, hw = (W + 1) >> 1;
+    for (int i = gtid; i < hw * H; i += nthreads) {              // two adjacent fine pixels per thread
+        const int y = i / hw, x = 2 * (i - y * hw);
+        const int x0 = x >> 1, x1 = min(x0 + 1, Wc - 1), y0 = y >> 1, y1 = min(y0 + 1, Hc - 1);
+        const float fy = (y & 1) * 0.5f;
+        const float a00 = __ldcg(C.u + y0 * cp + x0), a01 = __ldcg(C.u + y0 * cp + x1);
+        const float a10 = __ldcg(C.u + y1 * cp + x0), a11 = __ldcg(C.u + y1 * cp + x1);
+        const float b00 = __ldcg(C.v + y0 * cp + x0), b01 = __ldcg(C.v + y0 * cp + x1);
+        const float b10 = __ldcg(C.v + y1 * cp + x0), b11 = __ldcg(C.v + y1 * cp + x1);
+        // even x: fx = 0; odd x (= x+1): fx = 1/2
+        const float ue = 2.0f * ((1.0f - fy) * a00 + fy * a10);
+        const float ve = 2.0f * ((1.0f - fy) * b00 + fy * b10);
+        const float uo = 2.0f * ((1.0f - fy) * (0.5f * a00 + 0.5f * a01) + fy * (0.5f * a10 + 0.5f * a11));
+        const float vo = 2.0f * ((1.0f - fy) * (0.5f * b00 + 0.5f * b01) + fy * (0.5f * b10 + 0.5f * b11));
+        float *pu = F.u + y * F.pitch + x, *pv = F.v + y * F.pitch + x;
+        if (x + 1 < W) {
+            *reinterpret_cast<float2 *>(pu) = make_float2(ue, uo);
+            *reinterpret_cast<float2 *>(pv) = make_float2(ve, vo);
+        } else {
+            *pu = ue;
+            *pv = ve;
+        }
+    }
+}
+
+template <int R>
+__global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const SolveArgs a)
+{
+    extern __shared__ __align__(1024) unsigned char solve_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int cta = blockIdx.x, ncta = gridDim.x;
+    const K3Smem sm(solve_smem);
+    if (threadIdx.x == 0) k3_init_barriers<R>(sm);
+    __syncthreads();
+
+    uint32_t gc0 = 0;                                            // ring chunks consumed so far by this CTA
+    unsigned nbar = 0;                                           // grid barriers passed so far
+    int pi = 0;
+    prof_stamp(a, pi);
+    const int top = a.levels - 1;
+    for (int l = top; l >= 0; --l) {
+        const LevelDesc L = a.lv[l];
+        if (l < top) {
+            upsample_phase(L, a.lv[l + 1], cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
+            prof_stamp(a, pi);
+            if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
+            prof_stamp(a, pi);
+        }
+        K2Params p2 = {L.pyr[a.s1], L.pyr[a.s2], L.u, L.v, a.S, a.plane, L.W, L.H, L.pitch,
+                       L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, a.dbg};
+        for (int it = 0; it < a.iterations; ++it) {
+            // ---- K2 pass: warp + gradients + products + horizontal sums -> five planes
+            k2_phase<R>(p2, solve_smem, sm.counter + 1, warp, lane, cta, ncta);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            prof_stamp(a, pi);
+            if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
+            prof_stamp(a, pi);
+            // ---- K3 pass: vertical sums + solve + update
+            const bool last = (l == 0 && it == a.iterations - 1);
+            K3Params p3 = {L.u, L.v, last ? a.u_out : L.u, last ? a.v_out : L.v, last ? a.valid : nullptr, last ? a.det : nullptr,
+                           L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, a.dbg};
+            if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async;" ::: "memory");
+            k3_phase<R>(a.tm + l, p3, sm, warp, lane, SOLVE_WARPS - 1, cta, ncta, gc0);
+            gc0 += (uint32_t)k3_cta_chunks<R>(p3, cta, ncta);
+            __syncthreads();
+            if (threadIdx.x == 0) { sm.counter[0] = 0; sm.counter[1] = 0; }
+            prof_stamp(a, pi);
+            if (!last) { if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads(); }
+            prof_stamp(a, pi);
+        }
+    }
+    grid_barrier_exit(a.gbar, ncta);
+}

@@ -5,8 +5,7 @@
 // reach the GPU returns an error.
 #include "../../include/optflow.h"
 #include "of_kernels.cuh"
-#include "of_k2.cuh"
-#include "of_k3.cuh"
+#include "of_solve.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -98,6 +97,12 @@ struct of_context {
     K2Plan k2[OF_MAX_LEVELS];
     K3Plan k3[OF_MAX_LEVELS];
     CUtensorMap tmS[OF_MAX_LEVELS];     // the five summed planes of a level as one (x, y, field) tensor
+    LevelDesc *d_lv;                    // device copies for the persistent solve kernel
+    CUtensorMap *d_tm;
+    unsigned *d_gbar;
+    unsigned long long *d_prof;         // timeline buffer of the persistent kernel (of_solve_timeline)
+    bool prof_on;
+    bool persistent;                    // whole solve in one cooperative launch (default) vs one launch per kernel
     bool use_graph;
     std::vector<GraphEntry> graphs;
     unsigned long long stamp;
@@ -115,43 +120,44 @@ template <int R> int setup_attrs()
 {
     CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
 }
 
-// K2: warp tiles of (8*nseg) x (2*nrp) outputs, one CTA of `warps` independent warps per SM.  The
-// model below only ranks candidates: issue-bound time per SM vs the serial latency of one warp.
+// K2: warp tiles of (8*nseg) x (2*nrp) outputs; every CTA owns an equal range of tiles and its
+// SOLVE_WARPS warps pull from it.  The model only ranks candidates: the serial latency of the warp
+// that runs the most tiles (coarse levels: prefer one-round tiles with field-parallel sums) against
+// the instruction-issue time of the SM (fine levels: prefer wide tiles, less halo recomputation).
 template <int R> K2Plan plan_k2(int W, int H, int sms)
 {
     typedef K2Geom<R> G;
     K2Plan best = {};
     double best_cost = 1e30;
-    int f_nseg = 0, f_nrp = 0, f_wps = 0;
-    if (const char *e = getenv("OF_K2_GEOM")) sscanf(e, "%d,%d,%d", &f_nseg, &f_nrp, &f_wps);
+    int f_nseg = 0, f_nrp = 0;
+    if (const char *e = getenv("OF_K2_GEOM")) sscanf(e, "%d,%d", &f_nseg, &f_nrp);
     const int segs = (W + 7) / 8;
     for (int nrp = 1; nrp <= 4; nrp *= 2) {
         const int nsegmax = 32 / nrp, tx_min = (segs + nsegmax - 1) / nsegmax;
-        for (int tx = tx_min; tx <= tx_min + 3; ++tx) {
+        int last_nseg = 0;
+        for (int tx = tx_min; tx <= segs; ++tx) {
             int nseg = (segs + tx - 1) / tx;
-            if (f_nseg) { if (nrp != f_nrp) continue; nseg = std::min(f_nseg, nsegmax); }
+            if (f_nseg) { if (nrp != f_nrp) break; nseg = std::min(f_nseg, nsegmax); }
+            if (nseg == last_nseg) continue;
+            last_nseg = nseg;
             const int txr = (segs + nseg - 1) / nseg;
             const int tasks = G::pw(nseg) / 2 * nrp, rounds = (tasks + 31) / 32;
             const int ty = (H + 2 * nrp - 1) / (2 * nrp), ntiles = txr * ty;
             const int wb = G::warp_bytes(nseg, nrp);
-            const int wmax = std::min(16, SMEM_MAX / wb);
-            for (int wps = 1; wps <= wmax; ++wps) {
-                if (f_wps && wps != f_wps) continue;
-                const int per = (ntiles + sms * wps - 1) / (sms * wps);
-                const double tile_instr = rounds * 250.0 + 1250.0;
-                const double lat = per * (rounds * 1500.0 + 2300.0);
-                const int conc = std::min(wps, (ntiles + sms - 1) / sms);
-                const double ipc = std::min(2.4, 0.35 * conc);
-                const double thr = (double)per * wps * tile_instr / ipc;
-                const double cost = std::max(lat, thr);
-                if (cost < best_cost) {
-                    best_cost = cost;
-                    const int w = std::max(1, std::min(wps, (ntiles + sms - 1) / sms));
-                    best = {nseg, nrp, ty, ntiles, std::min(sms, (ntiles + w - 1) / w), w, w * wb};
-                }
+            if (SOLVE_WARPS * wb > K3_RING * K3_CHUNK_BYTES) { if (f_nseg) break; continue; }   // must fit under the K3 barriers
+            const int hs = (5 * nseg * nrp <= 32) ? 1 : 5;                 // serial field sums per lane
+            const int tiles_cta = (ntiles + sms - 1) / sms;
+            const int per = (tiles_cta + SOLVE_WARPS - 1) / SOLVE_WARPS;
+            const double lat = per * (rounds * 1400.0 + hs * 450.0 + 800.0);
+            const double thr = tiles_cta * (rounds * 380.0 + 5 * 290.0) / (4 * 0.8);
+            const double cost = std::max(lat, thr);
+            if (cost < best_cost) {
+                best_cost = cost;
+                best = {nseg, nrp, ty, ntiles, sms, SOLVE_WARPS, SOLVE_WARPS * wb};
             }
             if (f_nseg) break;
         }
@@ -165,10 +171,8 @@ template <int R> K3Plan plan_k3(int W, int H, int sms)
     K3Plan p = {};
     p.nrb = (H + 7) / 8;
     p.ntasks = ((W + 63) / 64) * p.nrb;
-    p.grid = std::min(sms, p.ntasks);
-    const int tpc = (p.ntasks + p.grid - 1) / p.grid;
-    p.warps = std::min(K3_MAX_NW, tpc);                         // consumer warps; one producer warp is added at launch
-    if (const char *e = getenv("OF_K3_NW")) { int v = atoi(e); if (v >= 1 && v <= K3_MAX_NW) p.warps = v; }
+    p.grid = sms;
+    p.warps = SOLVE_WARPS - 1;                                  // consumer warps; one producer warp is added at launch
     p.smem = K3Geom<R>::SMEM;
     return p;
 }
@@ -185,7 +189,7 @@ void launch_k2(const of_context *c, int l, const float *I1, const float *I2, cud
     const Level &L = c->lv[l];
     const K2Plan &P = c->k2[l];
     K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, P.ntiles, c->ww, c->dbg};
-    k2_products_hsum<R><<<P.grid, 32 * P.warps, P.smem, st>>>(p);
+    k2_products_hsum<R><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
 }
 
 template <int R>
@@ -196,6 +200,16 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
                   L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, c->dbg};
     k3_vsum_solve<R><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
+}
+
+template <int R>
+cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int s2, float *u_out, float *v_out, cudaStream_t st)
+{
+    SolveArgs a = {c->d_lv, c->d_tm, c->d_gbar, c->S, c->plane, u_out, v_out, c->valid, c->det,
+                   c->levels, c->iterations, s1, s2, c->W, c->dbg, c->prof_on ? c->d_prof : nullptr, c->ww, {0.5f * c->eps_rel, c->max_step}};
+    void *args[] = {&a};
+    return cudaLaunchCooperativeKernel((const void *)of_solve_pair<R>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
+                                       (size_t)K3Geom<R>::SMEM, st);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency:
@@ -302,6 +316,13 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
     cudaMemsetAsync(c->u[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
     cudaMemsetAsync(c->v[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
     note_launch(c, "memset", top);
+    if (c->persistent) {
+        cudaError_t e = cudaSuccess;
+        DISPATCH_R(c->R, e = launch_solve<R>(c, nullptr, j.s1, j.s2, j.u_out, j.v_out, st));
+        if (e != cudaSuccess && c->launch_err.empty()) c->launch_err = std::string("solve (persistent): ") + cudaGetErrorString(e);
+        note_launch(c, "solve (persistent)", 0);
+        return n + 1;
+    }
     for (int l = top; l >= 0; --l) {
         if (l < top) { run_upsample(c, l, st); note_launch(c, "upsample", l); ++n; }
         for (int it = 0; it < c->iterations; ++it) {
@@ -499,6 +520,23 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         c->dbg = getenv("OF_KERNEL_DEBUG") ? atoi(getenv("OF_KERNEL_DEBUG")) : 0;
         for (int l = 0; l < levels; ++l) { DISPATCH_R(window_radius, plan_level<R>(c, l)); }
         rc = encode_tensor_maps(c);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_lv, sizeof(LevelDesc) * levels);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_tm, sizeof(CUtensorMap) * levels);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_gbar, 256);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_prof, sizeof(unsigned long long) * OF_TIMELINE_MAX * c->sms);
+        if (rc == OF_OK) {
+            LevelDesc hl[OF_MAX_LEVELS];
+            for (int l = 0; l < levels; ++l)
+                hl[l] = {{c->pyr[0][l], c->pyr[1][l]}, c->u[l], c->v[l], lv[l].W, lv[l].H, lv[l].pitch,
+                         c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks};
+            cudaMemcpy(c->d_lv, hl, sizeof(LevelDesc) * levels, cudaMemcpyHostToDevice);
+            cudaMemcpy(c->d_tm, c->tmS, sizeof(CUtensorMap) * levels, cudaMemcpyHostToDevice);
+            cudaMemset(c->d_gbar, 0, 256);
+            if (cudaDeviceSynchronize() != cudaSuccess) rc = fail(OF_ERR_CUDA, "descriptor upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+            int coop = 0;
+            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+            c->persistent = coop != 0 && !(getenv("OF_PERSISTENT") && atoi(getenv("OF_PERSISTENT")) == 0);
+        }
         if (getenv("OF_DEBUG"))
             for (int l = 0; l < levels; ++l)
                 fprintf(stderr, "[optflow] level %d %dx%d pitch %d | K2 nseg %d nrp %d tiles %d grid %d warps %d smem %d | K3 tasks %d grid %d warps %d smem %d\n",
@@ -549,6 +587,40 @@ int of_set_graph(of_handle h, int enable)
     h->use_graph = enable != 0;
     if (!h->use_graph) drop_graphs(h);
     return OF_OK;
+}
+
+int of_set_persistent(of_handle h, int enable)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    h->persistent = enable != 0;
+    drop_graphs(h);
+    return OF_OK;
+}
+
+int of_solve_timeline(of_handle h, int enable, int cta, unsigned long long *out_host, int max_entries)
+{
+    static_assert(OF_TIMELINE_MAX == SOLVE_TIMELINE_MAX, "timeline sizes out of sync");
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    const int n = 1 + 2 * (h->levels - 1) + 4 * h->levels * h->iterations;
+    if (n > OF_TIMELINE_MAX) return fail(OF_ERR_INVALID_ARG, "timeline of %d entries exceeds OF_TIMELINE_MAX", n);
+    if (cta >= h->sms) return fail(OF_ERR_INVALID_ARG, "cta must be < %d", h->sms);
+    int got = 0;
+    if (out_host && h->prof_on) {
+        CU_TRY(cudaSetDevice(h->device));
+        CU_TRY(cudaDeviceSynchronize());
+        got = std::min(n, max_entries);
+        std::vector<unsigned long long> all((size_t)OF_TIMELINE_MAX * h->sms);
+        CU_TRY(cudaMemcpy(all.data(), h->d_prof, sizeof(unsigned long long) * all.size(), cudaMemcpyDeviceToHost));
+        // stamps are SM cycle counts: make them relative to each CTA's first stamp (CTAs start within ~1 us)
+        for (int i = 0; i < got; ++i) {
+            unsigned long long v = 0;
+            for (int c = (cta >= 0 ? cta : 0); c < (cta >= 0 ? cta + 1 : h->sms); ++c)
+                v = std::max(v, all[(size_t)c * OF_TIMELINE_MAX + i] - all[(size_t)c * OF_TIMELINE_MAX]);
+            out_host[i] = v;
+        }
+    }
+    if ((enable != 0) != h->prof_on) { h->prof_on = enable != 0; drop_graphs(h); }
+    return got;
 }
 
 int of_get_validity(of_handle h, uint8_t *mask_dev, void *stream)

@@ -288,7 +288,7 @@ def test_graph_and_plain_launches_agree_bitwise_and_repeat(torch, B):
     a = gpu_solve(torch, B, c.I1, c.I2, 3, 12, 4, GAUSS, graph=True)
     b = gpu_solve(torch, B, c.I1, c.I2, 3, 12, 4, GAUSS, graph=False)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
-    assert a[3] == b[3] == 1 + 2 + 2 + 3 * 4 * 2          # convert, 2 pyramid steps, 2 upsamples, 24 iteration kernels
+    assert a[3] == b[3] == 1 + 2 + 1                      # convert, 2 pyramid steps, 1 persistent solve
     H, W = c.I1.shape
     with B.OpticalFlow(W, H, 3, 12, 4, GAUSS) as of:
         d1, d2 = torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()
@@ -300,6 +300,27 @@ def test_graph_and_plain_launches_agree_bitwise_and_repeat(torch, B):
             u3, v3 = of.compute(d1, d2, u2, v2)   # same pointers: cached graph
         s.synchronize()
         assert torch.equal(u1, u2) and torch.equal(u1, u3) and np.array_equal(u1.cpu().numpy(), a[0])
+
+
+@pytest.mark.parametrize("W,H,L,R,it,wt", [(320, 256, 3, 12, 4, GAUSS), (130, 70, 2, 4, 3, BOX), (1280, 1024, 3, 12, 10, GAUSS)])
+def test_persistent_and_per_kernel_launches_agree_bitwise(torch, B, W, H, L, R, it, wt):
+    """The persistent solve kernel runs the same passes as the stand-alone K2/K3/K4 launches, so the two
+    modes must agree bit for bit (also pins the grid barrier and the cross-pass memory ordering)."""
+    c = syn.config3(W, H)
+    d1, d2 = torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()
+    out = []
+    for persistent in (True, False):
+        with B.OpticalFlow(W, H, L, R, it, wt) as of:
+            of.set_persistent(persistent)
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                for _ in range(3):                      # repeat: barrier generation and ring parity carry over
+                    u, v = of.compute(d1, d2)
+                m = of.validity()
+            s.synchronize()
+            out.append((u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy(), of.last_launch_count()))
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2])
+    assert out[0][3] == 1 + (L - 1) + 1 and out[1][3] == 1 + 2 * (L - 1) + 2 * L * it
 
 
 def test_large_image_crop_parity(torch, B, oracle):

@@ -6,8 +6,8 @@
         --master-port P bench.py --gpus N --steps K --warmup W
     python bench.py --impl reference ...      # the fp64 oracle on the host cores (slow on purpose)
 
-A "step" is one pass of the whole hot path (convert, pyramid, 3 levels x 10 iterations x {K2, K3},
-upsampling) over one frame pair of the workload `config3` (BASELINE.json:9; 1280x1024 uint8, 3 levels,
+A "step" is one pass of the whole hot path (convert, pyramid, then the persistent solve kernel: 3 levels
+x 10 iterations x {K2 pass, K3 pass} + flow hand-down) over one frame pair of the workload `config3` (BASELINE.json:9; 1280x1024 uint8, 3 levels,
 Gaussian window sigma 4 = radius 12, 10 iterations).  Frame pairs are independent, so
 N > 1 runs N replicas with no data-path collective ("replicas only", weak scaling).
 
@@ -34,6 +34,7 @@ METRIC = "dense-flow frame pairs/s at 1280x1024"
 UNIT = "pairs/s"
 WORKLOAD = "config3: 1280x1024 uint8 particle pair, backward-facing-step-like field, 3 levels, Gaussian window sigma 4 (R=12), 10 iterations"
 BYTES_PER_PX = {"k2_products_hsum": 16 + 20, "k3_vsum_solve": 28 + 8}    # 72 B per pixel-iteration
+NCU_DRAM_BYTES_PER_SOLVE = 14.49e6 + 9.56e6   # dram__bytes_read.sum + dram__bytes_write.sum, one of_solve_pair launch (profiles/)
 RING = 16          # default: distinct input pairs + output buffers cycled through: 16*(2.6+10.5) MB = 210 MB > 126 MB L2
 
 
@@ -58,7 +59,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -199,7 +200,18 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     launches = of.last_launch_count() * args.steps
 
-    # ---------------- dominant-kernel roofline (level 0), events on the launching stream
+    # ---------------- dominant kernel = the persistent solve kernel (all levels x iterations of a pair in one
+    # launch): CUDA events on the launching stream around `rep` back-to-back launches of that kernel alone
+    with torch.cuda.stream(stream):
+        of.run_solve(5)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        rep = 100
+        a.record()
+        of.run_solve(rep)
+        b.record()
+        b.synchronize()
+        solve_us = a.elapsed_time(b) / rep * 1e3
+    # stand-alone K2 / K3 launches at level 0 (each includes a kernel boundary, which the persistent kernel avoids)
     kt = {}
     with torch.cuda.stream(stream):
         for which, name in ((0, "k2_products_hsum"), (1, "k3_vsum_solve")):
@@ -211,6 +223,12 @@ def run_ours(args):
             b.record()
             b.synchronize()
             kt[name] = a.elapsed_time(b) / rep * 1e3      # us per launch
+    # in-kernel timeline (SM cycles at every pass boundary, max over CTAs) of one more solve
+    of.solve_timeline(True)
+    with torch.cuda.stream(stream):
+        of.compute(d_in[0][0], d_in[0][1], d_out[0][0], d_out[0][1])
+    stream.synchronize()
+    tl = of.solve_timeline(False).astype(np.float64)
     clocks = sampler.stop()
     ms = reduce_max_time(ms, dist, dev)
 
@@ -264,9 +282,18 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = measured_peaks()
         px = W * H
-        dom = max(kt, key=lambda k: kt[k])
-        ach = BYTES_PER_PX[dom] * px / (kt[dom] * 1e-6) / 1e9
-        iter_gbs = 72.0 * px / ((kt["k2_products_hsum"] + kt["k3_vsum_solve"]) * 1e-6) / 1e9
+        level_px = [((W + (1 << l) - 1) >> l) * ((H + (1 << l) - 1) >> l) for l in range(c0.levels)]
+        solve_bytes = 72.0 * sum(level_px) * c0.iterations
+        ach = solve_bytes / (solve_us * 1e-6) / 1e9
+        # level-0 iteration from the in-kernel timeline: {K2 pass, barrier, K3 pass, barrier} medians
+        mhz = clocks.get("sm_mhz") or 1965.0
+        L, it = c0.levels, c0.iterations
+        d = np.diff(tl) / mhz                                  # us per phase
+        i0 = 2 * (L - 1) + 4 * it * (L - 1)                    # first phase of level 0's iterations
+        seg = d[i0:i0 + 4 * it].reshape(it, 4)
+        med = np.median(seg[:-1], axis=0)
+        iter_us = float(med.sum())
+        iter_gbs = 72.0 * px / (iter_us * 1e-6) / 1e9
         pix_iters = sum(((W + (1 << l) - 1) >> l) * ((H + (1 << l) - 1) >> l) for l in range(c0.levels)) * c0.iterations
         value = world * args.steps / (ms * 1e-3)
         out = {
@@ -283,12 +310,16 @@ def run_ours(args):
                     "d2h_bytes_per_step": 8 * px, "steps": e2e_steps,
                     "api": "of_stream_open(PAIRS, host results) / acquire+fill / submit / result", "checksum": checksum},
             "gpu_launches": launches,
-            "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                         "traffic": None, "peak_source": peak_src, "bytes_per_launch": BYTES_PER_PX[dom] * px,
-                         "us_per_launch": kt[dom]},
-            "kernels_level0_us": kt,
-            "iteration_level0": {"bytes": 72 * px, "us": kt["k2_products_hsum"] + kt["k3_vsum_solve"], "GB/s": iter_gbs,
-                                 "frac_of_peak": iter_gbs / peak},
+            "roofline": {"bound": "hbm", "kernel": "of_solve_pair<12> (persistent: K2 pass + K3 pass + hand-down, all levels and iterations)",
+                         "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                         "traffic": NCU_DRAM_BYTES_PER_SOLVE, "traffic_source": "profiles/r1_persistent_solve.md (ncu --set full, dram read + write of one launch; the 47 MB of planes are L2 resident)",
+                         "peak_source": peak_src, "bytes_per_launch": solve_bytes,
+                         "bytes_basis": "72 B per pixel-iteration (K2 16 R + 20 W, K3 28 R + 8 W) x %d pixel-iterations" % (sum(level_px) * c0.iterations),
+                         "us_per_launch": solve_us},
+            "iteration_level0": {"bytes": 72 * px, "us": iter_us, "GB/s": iter_gbs, "frac_of_peak": iter_gbs / peak,
+                                 "phases_us": {"k2_pass": float(med[0]), "barrier_1": float(med[1]), "k3_pass": float(med[2]), "barrier_2": float(med[3])},
+                                 "how": "in-kernel SM cycle stamps (of_solve_timeline, max over CTAs) / sampled SM clock; median over iterations"},
+            "kernels_level0_standalone_us": kt,
             "cpu_baseline": cpu,
         }
         print(json.dumps(out))
@@ -301,7 +332,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -115,6 +115,11 @@ int of_get_debug_plane(of_handle h, int level, int which, float *out_dev, void *
  *   in place on the internal field). */
 int of_run_step(of_handle h, int level, int which, int repeat, void *stream);
 
+/* Launch ONLY the persistent solve kernel (plus the two memsets of the coarsest field), `repeat` times,
+ * on the pyramids left by the last of_compute*; the level-0 result is discarded into scratch.  For
+ * timing the dominant kernel with CUDA events and for ncu. */
+int of_run_solve(of_handle h, int repeat, void *stream);
+
 /* Timeline of the persistent solve kernel (profiling hook; the in-kernel analogue of a launch list).
  * While the hook is on, thread 0 of every CTA stores its SM cycle counter, relative to the CTA's start,
  * at every phase boundary (after a CTA-wide barrier; %globaltimer is refreshed too coarsely): start; per level coarse-to-fine { hand-down end, grid barrier end } (not for the

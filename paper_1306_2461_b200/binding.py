@@ -37,6 +37,7 @@ SIGNATURES = {
     "of_last_launch_count": (_i, [_vp]),
     "of_get_debug_plane": (_i, [_vp, _i, _i, _vp, _vp]),
     "of_run_step": (_i, [_vp, _i, _i, _i, _vp]),
+    "of_run_solve": (_i, [_vp, _i, _vp]),
     "of_pyramid_down": (_i, [_vp, _i, _i, _vp, _vp]),
     "of_upsample_flow": (_i, [_vp, _vp, _i, _i, _vp, _vp, _i, _i, _vp]),
     "of_stream_open": (_i, [_vp, _i, _i, _i]),
@@ -182,6 +183,9 @@ class OpticalFlow:
 
     def run_step(self, level, which, repeat=1, stream=None):
         _check(lib().of_run_step(self._h, level, which, repeat, _stream_ptr(stream)))
+
+    def run_solve(self, repeat=1, stream=None):
+        _check(lib().of_run_solve(self._h, repeat, _stream_ptr(stream)))
 
     # -- frame pipeline -----------------------------------------------------------------------
     def stream_open(self, dtype, mode=OF_STREAM_CONSECUTIVE, result_on_host=True):

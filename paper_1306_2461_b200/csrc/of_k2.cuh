@@ -155,9 +155,9 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
     const int W = p.W, H = p.H, pitch = p.pitch;
     const int ntasks = half * nrp;
     const int TW = 8 * nseg, TH = 2 * nrp;
-    // phase-2 role of this lane: (field group, row pair, segment).  Small tiles (5*nseg*nrp <= 32) give
-    // every field its own lanes, which shortens the serial chain of a coarse-level pass five-fold.
-    const int nf_par = (5 * nseg * nrp <= 32) ? 5 : 1;
+    // phase-2 role of this lane: (field group, row pair, segment).  Narrow tiles leave lanes free, so
+    // up to five fields are summed side by side, which shortens the serial chain of a coarse-level pass.
+    const int nf_par = max(1, min(5, 32 / (nseg * nrp)));
     const int h_seg = lane % nseg, h_rp = (lane / nseg) % nrp, h_f0 = lane / (nseg * nrp);
 
     const int t_begin = (int)((long long)p.ntiles * cta / ncta), t_end = (int)((long long)p.ntiles * (cta + 1) / ncta);

@@ -149,7 +149,8 @@ template <int R> K2Plan plan_k2(int W, int H, int sms)
             const int ty = (H + 2 * nrp - 1) / (2 * nrp), ntiles = txr * ty;
             const int wb = G::warp_bytes(nseg, nrp);
             if (SOLVE_WARPS * wb > K3_RING * K3_CHUNK_BYTES) { if (f_nseg) break; continue; }   // must fit under the K3 barriers
-            const int hs = (5 * nseg * nrp <= 32) ? 1 : 5;                 // serial field sums per lane
+            const int nf_par = std::max(1, std::min(5, 32 / (nseg * nrp)));
+            const int hs = (5 + nf_par - 1) / nf_par;                      // serial field sums per lane
             const int tiles_cta = (ntiles + sms - 1) / sms;
             const int per = (tiles_cta + SOLVE_WARPS - 1) / SOLVE_WARPS;
             const double lat = per * (rounds * 1400.0 + hs * 450.0 + 800.0);
@@ -664,6 +665,25 @@ int of_run_step(of_handle h, int level, int which, int repeat, void *stream)
         else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, (cudaStream_t)stream);
     }
     CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+int of_run_solve(of_handle h, int repeat, void *stream)
+{
+    if (!h || repeat < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    if (!h->persistent) return fail(OF_ERR_STATE, "persistent mode is off");
+    CU_TRY(cudaSetDevice(h->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int top = h->levels - 1;
+    const size_t top_bytes = sizeof(float) * (size_t)h->lv[top].pitch * h->lv[top].H;
+    for (int i = 0; i < repeat; ++i) {
+        CU_TRY(cudaMemsetAsync(h->u[top], 0, top_bytes, st));
+        CU_TRY(cudaMemsetAsync(h->v[top], 0, top_bytes, st));
+        cudaError_t e = cudaSuccess;
+        // the level-0 result goes to the handle's own scratch (first two planes of S are free after the solve)
+        DISPATCH_R(h->R, e = launch_solve<R>(h, nullptr, 0, 1, h->S + 3 * h->plane, h->S + 4 * h->plane, st));
+        if (e != cudaSuccess) return fail(OF_ERR_CUDA, "solve launch failed: %s", cudaGetErrorString(e));
+    }
     return OF_OK;
 }
 

@@ -140,13 +140,13 @@ __device__ __forceinline__ void k2_task_products(const K2Params &p, const K2In &
                 o[0].w, o[1].w, o[2].w, o[3].w, o[4].w);
 }
 
-// One K2 pass over a level by CTA `cta` of `ncta`: the CTA owns an equal, contiguous range of warp
-// tiles and its warps pull tiles from `tile_counter` (shared memory, 0 on entry, CTA-synchronised), so
+// One K2 pass over a level by one CTA: it owns the contiguous range [t_begin, t_end) of warp tiles
+// (cta_range) and its warps pull tiles from `tile_counter` (shared memory, 0 on entry, CTA-synchronised), so
 // fast warps take more tiles.  Which warp computes a tile does not change its arithmetic.  `smem_cta`
 // is the CTA's dynamic shared memory, of which this warp uses slice `warp`.  Called by the stand-alone
 // kernel below and by the persistent solve kernel (of_solve.cuh).
 template <int R>
-__device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_cta, int *tile_counter, int warp, int lane, int cta, int ncta)
+__device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_cta, int *tile_counter, int warp, int lane, int t_begin, int t_end)
 {
     typedef K2Geom<R> G;
     const int nseg = p.nseg, nrp = p.nrp;
@@ -160,7 +160,6 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
     const int nf_par = max(1, min(5, 32 / (nseg * nrp)));
     const int h_seg = lane % nseg, h_rp = (lane / nseg) % nrp, h_f0 = lane / (nseg * nrp);
 
-    const int t_begin = (int)((long long)p.ntiles * cta / ncta), t_end = (int)((long long)p.ntiles * (cta + 1) / ncta);
     for (;;) {
         int t = 0;
         if (lane == 0) t = atomicAdd(tile_counter, 1);
@@ -238,5 +237,7 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
                                                 (blockDim.x >> 5) * K2Geom<R>::warp_bytes(p.nseg, p.nrp));
     if (threadIdx.x == 0) *tile_counter = 0;
     __syncthreads();
-    k2_phase<R>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, blockIdx.x, gridDim.x);
+    int t_begin, t_end;
+    cta_range(p.ntiles, blockIdx.x, gridDim.x, t_begin, t_end);
+    k2_phase<R>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, t_begin, t_end);
 }

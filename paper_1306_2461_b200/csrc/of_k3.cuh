@@ -95,7 +95,9 @@ __device__ __forceinline__ void k3_solve_pair(float2 a, float2 b, float2 c, floa
     const float2 sq_ = __ffma2_rn(c, v, __ffma2_rn(b, u, q));       // -rq
     const float2 nu = sub2(__fmul2_rn(b, sq_), __fmul2_rn(C, sp_)); // C*rp - b*rq
     const float2 nv = sub2(__fmul2_rn(b, sp_), __fmul2_rn(A, sq_)); // A*rq - b*rp
-    const float2 inv = make_float2(__fdividef(1.0f, D.x), __fdividef(1.0f, D.y));
+    float2 inv;                                                 // MUFU.RCP, <= 1 ulp; D > 0 wherever tr > 0
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv.x) : "f"(D.x));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv.y) : "f"(D.y));
     du = __fmul2_rn(nu, inv);
     dv = __fmul2_rn(nv, inv);
     const float ms = sp.max_step;
@@ -127,21 +129,20 @@ template <int R> __device__ __forceinline__ void k3_init_barriers(const K3Smem &
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
 
-// Number of ring chunks CTA `cta` of `ncta` consumes in one K3 pass (uniform; advances the chunk base).
-template <int R> __device__ __forceinline__ int k3_cta_chunks(const K3Params &p, int cta, int ncta)
+// Number of ring chunks a CTA that owns tasks [t_begin, t_end) consumes in one K3 pass (advances the chunk base).
+template <int R> __device__ __forceinline__ int k3_cta_chunks(int t_begin, int t_end, int nrb)
 {
-    const int t_begin = (int)((long long)p.ntasks * cta / ncta), t_end = (int)((long long)p.ntasks * (cta + 1) / ncta);
     if (t_end <= t_begin) return 0;
-    return (t_end - t_begin) + ((t_end - 1) / p.nrb - t_begin / p.nrb + 1) * (K3Geom<R>::NC - 1);
+    return (t_end - t_begin) + ((t_end - 1) / nrb - t_begin / nrb + 1) * (K3Geom<R>::NC - 1);
 }
 
-// One K3 pass over a level by CTA `cta` of `ncta`.  Warp `nwc` (the last one) is the producer, warps
+// One K3 pass over a level by the CTA that owns tasks [t_begin, t_end) (cta_range).  Warp `nwc` (the last one) is the producer, warps
 // 0..nwc-1 consume.  `gc0` = number of ring chunks this CTA has consumed in earlier passes of the same
 // kernel (keeps slot / parity bookkeeping continuous); *sm.counter must be 0 on entry (CTA-synchronised).
 // All reads of u, v go through L2 (ld.global.cg): see of_k2.cuh.
 template <int R>
 __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params &p, const K3Smem &sm, int warp, int lane, int nwc,
-                                         int cta, int ncta, uint32_t gc0)
+                                         int t_begin, int t_end, uint32_t gc0)
 {
     typedef K3Geom<R> G;
     constexpr int NC = G::NC;
@@ -150,8 +151,6 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
     int *const counter = sm.counter;
     const int NWC = nwc;
     const int W = p.W, H = p.H, pitch = p.pitch, nrb = p.nrb;
-    const int t_begin = (int)((long long)p.ntasks * cta / ncta);
-    const int t_end = (int)((long long)p.ntasks * (cta + 1) / ncta);
     const int s_first = t_begin / nrb;
     // Task i of this CTA (global task t_begin+i in strip s) reads ring chunks gc0 + i + (s-s_first)*(NC-1) + k.
 
@@ -273,5 +272,7 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
     const K3Smem sm(k3_smem_);
     if (threadIdx.x == 0) k3_init_barriers<R>(sm);
     __syncthreads();
-    k3_phase<R>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, blockIdx.x, gridDim.x, 0u);
+    int t_begin, t_end;
+    cta_range(p.ntasks, blockIdx.x, gridDim.x, t_begin, t_end);
+    k3_phase<R>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, t_begin, t_end, 0u);
 }

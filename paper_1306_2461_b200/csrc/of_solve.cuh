@@ -31,9 +31,11 @@ struct LevelDesc {
     int k3_nrb, k3_ntasks;
 };
 
+#define SOLVE_MAX_LEVELS 12
 struct SolveArgs {
+    alignas(64) CUtensorMap tm[SOLVE_MAX_LEVELS];   // per level: the five planes as an (x, y, field) tensor; lives in
+                                                    // the kernel's parameter space (__grid_constant__), no global fetch
     const LevelDesc *lv;                     // device array [levels]
-    const CUtensorMap *tm;                   // device array [levels], 64-byte aligned
     unsigned *gbar;                          // {arrival count, generation}, zero-initialised once
     float *S;
     size_t plane;
@@ -117,7 +119,7 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
 }
 
 template <int R>
-__global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const SolveArgs a)
+__global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __grid_constant__ SolveArgs a)
 {
     extern __shared__ __align__(1024) unsigned char solve_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -139,11 +141,15 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const Solve
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
             prof_stamp(a, pi);
         }
+        int k2_b, k2_e, k3_b, k3_e;                              // this CTA's share of the level's tiles and tasks
+        cta_range(L.k2_ntiles, cta, ncta, k2_b, k2_e);
+        cta_range(L.k3_ntasks, cta, ncta, k3_b, k3_e);
+        const uint32_t k3_chunks = (uint32_t)k3_cta_chunks<R>(k3_b, k3_e, L.k3_nrb);
         K2Params p2 = {L.pyr[a.s1], L.pyr[a.s2], L.u, L.v, a.S, a.plane, L.W, L.H, L.pitch,
                        L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, a.dbg};
         for (int it = 0; it < a.iterations; ++it) {
             // ---- K2 pass: warp + gradients + products + horizontal sums -> five planes
-            k2_phase<R>(p2, solve_smem, sm.counter + 1, warp, lane, cta, ncta);
+            k2_phase<R>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             prof_stamp(a, pi);
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
@@ -153,8 +159,8 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const Solve
             K3Params p3 = {L.u, L.v, last ? a.u_out : L.u, last ? a.v_out : L.v, last ? a.valid : nullptr, last ? a.det : nullptr,
                            L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, a.dbg};
             if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async;" ::: "memory");
-            k3_phase<R>(a.tm + l, p3, sm, warp, lane, SOLVE_WARPS - 1, cta, ncta, gc0);
-            gc0 += (uint32_t)k3_cta_chunks<R>(p3, cta, ncta);
+            k3_phase<R>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            gc0 += k3_chunks;
             __syncthreads();
             if (threadIdx.x == 0) { sm.counter[0] = 0; sm.counter[1] = 0; }
             prof_stamp(a, pi);

@@ -206,8 +206,13 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
 template <int R>
 cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int s2, float *u_out, float *v_out, cudaStream_t st)
 {
-    SolveArgs a = {c->d_lv, c->d_tm, c->d_gbar, c->S, c->plane, u_out, v_out, c->valid, c->det,
-                   c->levels, c->iterations, s1, s2, c->W, c->dbg, c->prof_on ? c->d_prof : nullptr, c->ww, {0.5f * c->eps_rel, c->max_step}};
+    static_assert(SOLVE_MAX_LEVELS == OF_MAX_LEVELS, "level limits out of sync");
+    SolveArgs a;
+    memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
+    a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
+    a.valid = c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
+    a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
+    a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
     void *args[] = {&a};
     return cudaLaunchCooperativeKernel((const void *)of_solve_pair<R>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
                                        (size_t)K3Geom<R>::SMEM, st);

@@ -38,7 +38,7 @@ struct K2Params {
     int nseg, nrp;                                 // lane layout of a warp tile
     int tiles_y, ntiles;                           // tile t -> (tx = t / tiles_y, ty = t % tiles_y)
     WinWeights ww;
-    int dbg;                                       // profiling switches (0 in production): 1 = no product phase, 2 = no sum phase
+    int dbg;                                       // profiling switches (0 in production): 1 = no product phase, 2 = no sum phase, 32 = no plane stores
 };
 
 // Inputs of one phase-1 task (2 columns x 2 rows): I1 rows y-1..y+2 at columns x, x+1, the left and
@@ -212,7 +212,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
                 for (int tap = 0; tap <= 2 * R; ++tap)
 #pragma unroll
                     for (int j = 0; j < 8; ++j) acc[j] = fma2s(p.ww.w[tap], in[j + tap + G::OFF], acc[j]);
-                if (gx < pitch) {
+                if (gx < pitch && (!(p.dbg & 32) || acc[0].x == 12345.678f)) {
                     float *d0 = p.S + f * p.plane + (size_t)gy * pitch + gx;
                     if (gy < H) {
                         *reinterpret_cast<float4 *>(d0) = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);

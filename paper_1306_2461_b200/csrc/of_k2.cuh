@@ -50,51 +50,62 @@ struct K2In {
     float l0, q0, l1, q1;
 };
 
+// base + 4*idx as ONE IMAD.WIDE (FMA pipe).  The integer/compare pipe (16 lanes per clock per SM sub-partition)
+// is what bounds the product phase, so address arithmetic is kept off it.
+__device__ __forceinline__ const float *ptr_at(const float *base, int idx)
+{
+    const float *r;
+    asm("mad.wide.s32 %0, %1, 4, %2;" : "=l"(r) : "r"(idx), "l"(base));
+    return r;
+}
+
 __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
 {
     K2In in;
     const int W = p.W, H = p.H, pitch = p.pitch;
     const int i0 = y * pitch + x;                                  // one index, rows by +-pitch
     const int dm = y > 0 ? -pitch : 0, d1 = y + 1 < H ? pitch : 0, d2 = (y + 2 < H ? pitch : 0) + d1;
-    const float *c = p.I1 + i0, *c1p = c + d1;
-    in.cm = __ldg(reinterpret_cast<const float2 *>(c + dm));
+    const float *c = ptr_at(p.I1, i0), *c1p = ptr_at(c, d1);
+    in.cm = __ldg(reinterpret_cast<const float2 *>(ptr_at(c, dm)));
     in.c0 = __ldg(reinterpret_cast<const float2 *>(c));
     in.c1 = __ldg(reinterpret_cast<const float2 *>(c1p));
-    in.c2 = __ldg(reinterpret_cast<const float2 *>(c + d2));
-    const float *pu = p.u + i0, *pv = p.v + i0;
+    in.c2 = __ldg(reinterpret_cast<const float2 *>(ptr_at(c, d2)));
+    const float *pu = ptr_at(p.u, i0), *pv = ptr_at(p.v, i0);
     in.u0 = __ldcg(reinterpret_cast<const float2 *>(pu));
-    in.u1 = __ldcg(reinterpret_cast<const float2 *>(pu + d1));
+    in.u1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pu, d1)));
     in.v0 = __ldcg(reinterpret_cast<const float2 *>(pv));
-    in.v1 = __ldcg(reinterpret_cast<const float2 *>(pv + d1));
+    in.v1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pv, d1)));
     // left / right neighbours with clamp-to-edge: x-1 -> x at the left border, x+2 -> W-1 at the right
     const int ol = x > 0 ? -1 : 0, orr = x + 2 < W ? 2 : (x + 1 < W ? 1 : 0);
-    in.l0 = __ldg(c + ol);
-    in.q0 = __ldg(c + orr);
-    in.l1 = __ldg(c1p + ol);
-    in.q1 = __ldg(c1p + orr);
+    in.l0 = __ldg(ptr_at(c, ol));
+    in.q0 = __ldg(ptr_at(c, orr));
+    in.l1 = __ldg(ptr_at(c1p, ol));
+    in.q1 = __ldg(ptr_at(c1p, orr));
     return in;
 }
 
 // Bilinear sample of I2 at (x+u, y+v) (D8: the integer part of the displacement is added to the
-// integer pixel index; x+u is never formed in fp32).  Clamp-to-edge is applied as: clamp the cell
-// origin to [0, W-2] x [0, H-2] and force the fraction to 0 / 1 outside, which selects the same
-// pixels as clamping both taps (and is exact at the borders), with two row pointers + immediate
-// offsets instead of four separate addresses.  Split in two so that a lane can issue the gathers
-// of all its pixels before it consumes the first one.
+// pixel index; x+u is never formed in fp32).  Clamp-to-edge is applied as: clamp the cell origin to
+// [0, W-2] x [0, H-2] and force the fraction to 0 / 1 outside, which selects the same pixels as
+// clamping both taps (and is exact at the borders), with two row pointers + immediate offsets
+// instead of four separate addresses.  Split in two so that a lane can issue the gathers of all its
+// pixels before it consumes the first one.
 struct K2Tap { float i00, i01, i10, i11, ax, ay; };
 
-__device__ __forceinline__ K2Tap k2_gather(const float *__restrict__ I2, int x, int y, int Wm2, int Hm2, int pitch, float uu, float vv)
+// xf, yf = the pixel's coordinates as floats.  x + floor(u) is formed in fp32, which is exact (two integers
+// below 2^24); x + u never is (D8).  Clamping is done on that float: Xc = clamp(X, 0, W-2), and the
+// fraction becomes saturate(ax + (X - Xc)): unchanged inside, 0 left of the image, 1 right of it -- no
+// compare / select instructions.
+__device__ __forceinline__ K2Tap k2_gather(const float *__restrict__ I2, float xf, float yf, float Wm2f, float Hm2f, int pitch, float uu, float vv)
 {
     K2Tap t;
     const float fu = floorf(uu), fv = floorf(vv);
-    t.ax = uu - fu;
-    t.ay = vv - fv;
-    const int X = x + (int)fminf(fmaxf(fu, -65536.f), 65536.f);
-    const int Y = y + (int)fminf(fmaxf(fv, -65536.f), 65536.f);
-    t.ax = X < 0 ? 0.f : (X > Wm2 ? 1.f : t.ax);
-    t.ay = Y < 0 ? 0.f : (Y > Hm2 ? 1.f : t.ay);
-    const float *p0 = I2 + (max(0, min(Y, Hm2)) * pitch + max(0, min(X, Wm2)));
-    const float *p1 = p0 + pitch;
+    const float Xf = xf + fu, Yf = yf + fv;
+    const float Xc = fminf(fmaxf(Xf, 0.f), Wm2f), Yc = fminf(fmaxf(Yf, 0.f), Hm2f);
+    t.ax = __saturatef((uu - fu) + (Xf - Xc));
+    t.ay = __saturatef((vv - fv) + (Yf - Yc));
+    const float *p0 = ptr_at(I2, __float2int_rn(Yc) * pitch + __float2int_rn(Xc));
+    const float *p1 = ptr_at(p0, pitch);
     t.i00 = __ldg(p0); t.i01 = __ldg(p0 + 1); t.i10 = __ldg(p1); t.i11 = __ldg(p1 + 1);
     return t;
 }
@@ -110,11 +121,11 @@ __device__ __forceinline__ float k2_lerp(const K2Tap &t)
 // The four pixels of one phase-1 task: gathers first (k2_task_gather), products later (k2_task_products).
 __device__ __forceinline__ void k2_task_gather(const K2Params &p, const K2In &in, int x, int y, K2Tap (&t)[4])
 {
-    const int Wm2 = p.W - 2, Hm2 = p.H - 2;
-    t[0] = k2_gather(p.I2, x, y, Wm2, Hm2, p.pitch, in.u0.x, in.v0.x);
-    t[1] = k2_gather(p.I2, x, y + 1, Wm2, Hm2, p.pitch, in.u1.x, in.v1.x);
-    t[2] = k2_gather(p.I2, x + 1, y, Wm2, Hm2, p.pitch, in.u0.y, in.v0.y);
-    t[3] = k2_gather(p.I2, x + 1, y + 1, Wm2, Hm2, p.pitch, in.u1.y, in.v1.y);
+    const float Wm2f = (float)(p.W - 2), Hm2f = (float)(p.H - 2), xf = (float)x, yf = (float)y;
+    t[0] = k2_gather(p.I2, xf, yf, Wm2f, Hm2f, p.pitch, in.u0.x, in.v0.x);
+    t[1] = k2_gather(p.I2, xf, yf + 1.0f, Wm2f, Hm2f, p.pitch, in.u1.x, in.v1.x);
+    t[2] = k2_gather(p.I2, xf + 1.0f, yf, Wm2f, Hm2f, p.pitch, in.u0.y, in.v0.y);
+    t[3] = k2_gather(p.I2, xf + 1.0f, yf + 1.0f, Wm2f, Hm2f, p.pitch, in.u1.y, in.v1.y);
 }
 
 // It = I2w - I1 - Ix*u - Iy*v (D10) and the five products.  gx, gy are already multiplied by the

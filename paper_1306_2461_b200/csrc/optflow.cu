@@ -125,9 +125,8 @@ template <int R> int setup_attrs()
 }
 
 // K2: warp tiles of (8*nseg) x (2*nrp) outputs; every CTA owns an equal range of tiles and its
-// SOLVE_WARPS warps pull from it.  The model only ranks candidates: the serial latency of the warp
-// that runs the most tiles (coarse levels: prefer one-round tiles with field-parallel sums) against
-// the instruction-issue time of the SM (fine levels: prefer wide tiles, less halo recomputation).
+// SOLVE_WARPS warps pull from it.  The model only ranks candidates by the serial latency of a CTA's pass
+// (coarse levels: one-round tiles with field-parallel sums; fine levels: fewer, wider tiles).
 template <int R> K2Plan plan_k2(int W, int H, int sms)
 {
     typedef K2Geom<R> G;
@@ -151,11 +150,15 @@ template <int R> K2Plan plan_k2(int W, int H, int sms)
             if (SOLVE_WARPS * wb > K3_RING * K3_CHUNK_BYTES) { if (f_nseg) break; continue; }   // must fit under the K3 barriers
             const int nf_par = std::max(1, std::min(5, 32 / (nseg * nrp)));
             const int hs = (5 + nf_par - 1) / nf_par;                      // serial field sums per lane
+            // Serial latency of a CTA's pass, in SM cycles, fitted to the in-kernel timeline (profiles/
+            // r1_experiments.md): a tile costs 1850 + 1300 per product round + (550 + 400 x warps sharing a
+            // sub-partition's FMA pipe) per serial field sum; a CTA runs its tiles in waves of SOLVE_WARPS.
             const int tiles_cta = (ntiles + sms - 1) / sms;
-            const int per = (tiles_cta + SOLVE_WARPS - 1) / SOLVE_WARPS;
-            const double lat = per * (rounds * 1400.0 + hs * 450.0 + 800.0);
-            const double thr = tiles_cta * (rounds * 380.0 + 5 * 290.0) / (4 * 0.8);
-            const double cost = std::max(lat, thr);
+            double cost = 0.0;
+            for (int left = tiles_cta; left > 0; left -= SOLVE_WARPS) {
+                const int conc = std::min(left, SOLVE_WARPS);
+                cost += 1850.0 + rounds * 1300.0 + hs * (550.0 + 400.0 * ((conc + 3) / 4));
+            }
             if (cost < best_cost) {
                 best_cost = cost;
                 best = {nseg, nrp, ty, ntiles, sms, SOLVE_WARPS, SOLVE_WARPS * wb};

@@ -187,14 +187,25 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         const int gbase = (int)gc0 + i + (s - s_first) * (NC - 1);
         const int gx = 64 * s + 2 * lane, gy0 = 8 * rb;
         const bool active = gx < W;
+        // this lane's field values, issued before the waits (rows past the image re-read the last row)
+        const int nrows = min(8, H - gy0);
+        const float *ui = p.u_in + (size_t)gy0 * pitch + gx, *vi = p.v_in + (size_t)gy0 * pitch + gx;
+        float2 uu[8], vv[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int jj = min(j, nrows - 1) * pitch;
+            uu[j] = active ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
+            vv[j] = active ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
+        }
         const unsigned char *cb[NC];
-        uint32_t eb[NC];
+        uint32_t eb[NC], fb[NC], fpar[NC];
 #pragma unroll
         for (int k = 0; k < NC; ++k) {
             const int gc = gbase + k, slot = gc % K3_RING;
             cb[k] = k3_smem + slot * K3_CHUNK_BYTES + lane * 8;
             eb[k] = empty0 + 8 * slot;
-            if (!(p.dbg & 1)) mbar_wait(full0 + 8 * slot, (gc / K3_RING) & 1);
+            fb[k] = full0 + 8 * slot;
+            fpar[k] = (gc / K3_RING) & 1;
         }
         float2 acc[5][8];
 #pragma unroll
@@ -204,6 +215,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         if (!(p.dbg & 2))
 #pragma unroll
         for (int r = 0; r < G::NIN; ++r) {
+            if ((r & 7) == 0 && !(p.dbg & 1)) mbar_wait(fb[r >> 3], fpar[r >> 3]);   // chunk by chunk, as the TMA delivers them
 #pragma unroll
             for (int f = 0; f < 5; ++f) {
                 const float2 val = *reinterpret_cast<const float2 *>(cb[r >> 3] + f * 2048 + (r & 7) * 256);
@@ -218,21 +230,9 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             for (int k = 0; k < NC; ++k) mbar_arrive(eb[k], 1);
         }
         if (!active || (p.dbg & 4)) continue;
-        // ---- solve + update for 8 rows x 2 columns (field values are loaded here: TLP hides them)
-        const int nrows = min(8, H - gy0);
+        // ---- solve + update for 8 rows x 2 columns
         const bool pair_ok = gx + 1 < W;
         const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
-        const float *ui = p.u_in + (size_t)gy0 * pitch + gx, *vi = p.v_in + (size_t)gy0 * pitch + gx;
-        float2 uu[8], vv[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            uu[j] = make_float2(0.f, 0.f);
-            vv[j] = make_float2(0.f, 0.f);
-            if (j < nrows) {
-                uu[j] = __ldcg(reinterpret_cast<const float2 *>(ui + j * pitch));
-                vv[j] = __ldcg(reinterpret_cast<const float2 *>(vi + j * pitch));
-            }
-        }
         float *uo = p.u_out + (size_t)gy0 * p.out_pitch + gx, *vo = p.v_out + (size_t)gy0 * p.out_pitch + gx;
         float2 trs[8], dets[8];
 #pragma unroll

@@ -23,7 +23,9 @@
  * negation; window sums vs brute force on 32x32; transpose / mirror / gain-offset invariances;
  * reduction to textbook Lucas-Kanade (scipy uniform_filter); integer shift; pyramid and upsample
  * exactness on constants and ramps; eq. 1 behaviour; monotone error vs iterations
- * (Table 1 trend).  No function here is "parity unpinned".
+ * (Table 1 trend); oracle_equalise (eq. 2): zero local mean / unit local variance,
+ * gain-offset invariance, flat image -> 0, agreement with scipy uniform_filter in the interior.
+ * No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdlib.h>
@@ -290,6 +292,39 @@ int oracle_solve(const double *I1, const double *I2, int W, int H, int levels, i
     free(uc); free(vc);
     for (int l = 1; l < levels; ++l) { free(P1[l]); free(P2[l]); }
     return 0;
+}
+
+/* NEXT item f1: local equalisation pre-filter, eq. 2 of the paper:
+ *     In(x,y) = ( I(x,y) - mean(x,y) ) / sqrt( mean_of_squares(x,y) - mean(x,y)^2 )
+ * "where [the bar] is a local mean for a given radius.  We choose a radius of 5 pixels."  The printed
+ * denominator is garbled (D19); this is the zero-mean, unit-local-standard-deviation reading the text
+ * gives ("the mean intensity value is subtracted ... and divided by the local intensity standard
+ * deviation").  Readings: E1 the local mean is the plain average over the (2r+1)^2 box; E2 at the
+ * borders over the in-image part of the box (divided by the number of pixels actually summed), so
+ * a constant image has zero mean-removed value everywhere; E3 where the local variance is not
+ * positive (flat neighbourhood) the output is 0; E4 no rescaling afterwards (the solve is gain and
+ * offset invariant); E5 applied to both images before the pyramid.
+ * Plain double loops over the window, no running sums. */
+void oracle_equalise(const double *src, int W, int H, int r, double *dst)
+{
+#pragma omp parallel for
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            double s = 0.0, s2 = 0.0;
+            int n = 0;
+            for (int dy = -r; dy <= r; ++dy)
+                for (int dx = -r; dx <= r; ++dx) {
+                    int xx = x + dx, yy = y + dy;
+                    if (xx < 0 || xx >= W || yy < 0 || yy >= H) continue;
+                    double v = src[(size_t)yy * W + xx];
+                    s += v;
+                    s2 += v * v;
+                    ++n;
+                }
+            double mean = s / n;
+            double num = n * s2 - s * s;              /* n^2 * variance: exact for integer images */
+            dst[(size_t)y * W + x] = num > 0.0 ? (src[(size_t)y * W + x] - mean) / (sqrt(num) / n) : 0.0;
+        }
 }
 
 int oracle_num_threads(void)

@@ -75,6 +75,15 @@ def upsample_flow(coarse, W, H):
     return out
 
 
+def equalise(img, r=5):
+    """Local equalisation pre-filter, eq. 2."""
+    src, ps = _d(img)
+    H, W = src.shape
+    out = np.empty((H, W))
+    lib().oracle_equalise(ps, ctypes.c_int(W), ctypes.c_int(H), ctypes.c_int(r), out.ctypes.data_as(_dp))
+    return out
+
+
 def warp(I2, u, v):
     a, pa = _d(I2)
     uu, pu = _d(u)

@@ -373,3 +373,59 @@ def test_empty_windows_are_invalid_and_keep_zero_flow(oracle):
     # central differences of the 4x4 block are non-zero on a plus-shaped support inside rows/cols
     # 29..34 without its four corner pixels; dilated by the 9x9 window: 14x14 minus the 4 corners
     assert r["valid"].sum() == (6 + 8) ** 2 - 4
+
+
+# ---------------------------------------------------------------------------- eq. 2 (NEXT item f1)
+def test_equalise_matches_library_box_statistics_in_interior(oracle):
+    """eq. 2: (I - local mean) / local std over an 11x11 box; in the interior the
+    local moments are what scipy.ndimage.uniform_filter computes."""
+    from scipy.ndimage import uniform_filter
+    rng = np.random.default_rng(3)
+    I = rng.integers(0, 256, (48, 64)).astype(np.float64)
+    r = 5
+    out = oracle.equalise(I, r)
+    m = uniform_filter(I, 2 * r + 1, mode="constant")
+    m2 = uniform_filter(I * I, 2 * r + 1, mode="constant")
+    ref = (I - m) / np.sqrt(m2 - m * m)
+    sl = (slice(r, -r), slice(r, -r))
+    assert np.max(np.abs(out[sl] - ref[sl])) < 1e-10
+
+
+def test_equalise_borders_use_the_in_image_part_of_the_box(oracle):
+    rng = np.random.default_rng(4)
+    I = rng.integers(0, 4096, (20, 23)).astype(np.float64)
+    r = 3
+    out = oracle.equalise(I, r)
+    for (x, y) in ((0, 0), (22, 0), (0, 19), (22, 19), (1, 10), (11, 18)):
+        win = I[max(0, y - r):y + r + 1, max(0, x - r):x + r + 1]
+        ref = (I[y, x] - win.mean()) / win.std()
+        assert abs(out[y, x] - ref) < 1e-10, (x, y)
+
+
+def test_equalise_invariances_and_flat_guard(oracle):
+    rng = np.random.default_rng(5)
+    I = rng.integers(0, 256, (40, 40)).astype(np.float64)
+    a = oracle.equalise(I, 5)
+    b = oracle.equalise(3.5 * I + 17.0, 5)                    # illumination gain and offset drop out
+    assert np.max(np.abs(a - b)) < 1e-9
+    assert np.all(oracle.equalise(np.full((30, 30), 99.0), 5) == 0.0)     # flat -> 0, never NaN
+    flat = I.copy()
+    flat[10:30, 10:30] = 50.0
+    out = oracle.equalise(flat, 5)
+    assert np.isfinite(out).all() and np.all(out[15:25, 15:25] == 0.0)
+
+
+def test_flow_is_unchanged_by_equalisation_of_an_unevenly_lit_pair(oracle):
+    """Purpose of eq. 2: 'eliminate the influence of illumination inhomogeneities'.  A smooth
+    multiplicative illumination change between the frames biases the raw solve; after equalisation the
+    bias is gone (error vs the known shift drops)."""
+    d = (0.37, -0.21)
+    I1, I2 = syn.bandlimited_pair(192, 160, shift=d)
+    yy, xx = np.mgrid[0:160, 0:192]
+    lit = 1.0 + 0.4 * xx / 192.0 + 0.2 * yy / 160.0
+    raw = oracle.solve(I1, I2 * lit, 1, 10, 4, BOX)
+    eq = oracle.solve(oracle.equalise(I1, 5), oracle.equalise(I2 * lit, 5), 1, 10, 4, BOX)
+    m = (slice(24, -24), slice(24, -24))
+    err_raw = np.sqrt(np.mean((raw["u"][m] - d[0]) ** 2 + (raw["v"][m] - d[1]) ** 2))
+    err_eq = np.sqrt(np.mean((eq["u"][m] - d[0]) ** 2 + (eq["v"][m] - d[1]) ** 2))
+    assert err_eq < 0.5 * err_raw and err_eq < 0.05

@@ -81,6 +81,12 @@ const char *of_last_error(void);
  * eps_rel >= 0, max_step_px > 0. */
 int of_set_conditioning(of_handle h, float eps_rel, float max_step_px);
 
+/* Local equalisation pre-filter (eq. 2: "mandatory for experimental images"): every frame
+ * is replaced by (I - local mean) / local standard deviation over the in-image part of a (2*radius+1)^2
+ * box before the pyramid is built; 0 where the local variance is not positive.  Fused with the frame
+ * conversion (it replaces that kernel).  radius 0 (default) switches it off; the paper uses 5. */
+int of_set_equalisation(of_handle h, int radius);
+
 /* Replay the per-pair launch sequence as a CUDA graph (default on).  The graph is re-captured when
  * the caller's pointers change. */
 int of_set_graph(of_handle h, int enable);

@@ -29,6 +29,7 @@ SIGNATURES = {
     "of_compute_u16": (_i, [_vp] * 6),
     "of_last_error": (_c.c_char_p, []),
     "of_set_conditioning": (_i, [_vp, _c.c_float, _c.c_float]),
+    "of_set_equalisation": (_i, [_vp, _i]),
     "of_set_graph": (_i, [_vp, _i]),
     "of_set_persistent": (_i, [_vp, _i]),
     "of_solve_timeline": (_i, [_vp, _i, _i, _vp, _i]),
@@ -143,6 +144,9 @@ class OpticalFlow:
 
     def set_conditioning(self, eps_rel=1e-3, max_step_px=3.0):
         _check(lib().of_set_conditioning(self._h, eps_rel, max_step_px))
+
+    def set_equalisation(self, radius: int):
+        _check(lib().of_set_equalisation(self._h, int(radius)))
 
     def set_graph(self, enable: bool):
         _check(lib().of_set_graph(self._h, 1 if enable else 0))

@@ -1,0 +1,115 @@
+// of_equalise.cuh -- local equalisation pre-filter fused with the frame conversion (NEXT item f1 of the
+// scope table; eq. 2; readings E1-E5 in DESIGN.md):
+//     In(x,y) = (I - local mean) / local standard deviation   over the in-image part of a (2r+1)^2 box,
+//     0 where the local variance is not positive.
+// Replaces K0 when of_set_equalisation(h, r > 0): reads the raw uint8 / uint16 / float frame once and
+// writes the normalised fp32 level-0 plane.  CTA = 64 x 32 outputs; the raw patch with its halo is staged
+// in shared memory, then two separable box passes (rows, columns) of the sums of I and I^2.  Integer
+// frames are summed in integer arithmetic (uint32 / uint64), so n*sum(I^2) - sum(I)^2 is exact and the
+// flat-neighbourhood decision (variance > 0) is the same as the fp64 oracle's; float frames use fp64 sums.
+#pragma once
+#include "of_common.cuh"
+
+#define EQ_TW 64
+#define EQ_TH 32
+
+template <typename T> struct EqAcc { typedef unsigned int S1; typedef unsigned long long S2; };
+template <> struct EqAcc<uint8_t> { typedef unsigned int S1; typedef unsigned int S2; };       // 33^2 * 255^2 < 2^32
+template <> struct EqAcc<float> { typedef double S1; typedef double S2; };
+
+__host__ __device__ inline size_t eq_smem_bytes(int r, size_t elem)
+{
+    const size_t pw = EQ_TW + 2 * r, ph = EQ_TH + 2 * r;
+    return ph * pw * elem + ph * EQ_TW * (sizeof(unsigned long long) + sizeof(double));   // patch + row sums (upper bound)
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, const T *__restrict__ srcB,
+                                                   float *__restrict__ dstA, float *__restrict__ dstB,
+                                                   int W, int H, int pitch, int r)
+{
+    typedef typename EqAcc<T>::S1 S1;
+    typedef typename EqAcc<T>::S2 S2;
+    const T *__restrict__ src = blockIdx.z ? srcB : srcA;
+    float *__restrict__ dst = blockIdx.z ? dstB : dstA;
+    if (src == nullptr) return;
+    extern __shared__ __align__(16) unsigned char eq_smem[];
+    const int pw = EQ_TW + 2 * r, ph = EQ_TH + 2 * r;
+    S2 *h2 = reinterpret_cast<S2 *>(eq_smem);                         // [ph][EQ_TW] row sums of I^2
+    S1 *h1 = reinterpret_cast<S1 *>(h2 + (size_t)ph * EQ_TW);         // [ph][EQ_TW] row sums of I
+    T *patch = reinterpret_cast<T *>(h1 + (size_t)ph * EQ_TW);        // [ph][pw] raw values, 0 outside the image
+    const int x0 = blockIdx.x * EQ_TW, y0 = blockIdx.y * EQ_TH;
+    for (int i = threadIdx.x; i < ph * pw; i += 256) {
+        const int py = i / pw, px = i - py * pw;
+        const int gx = x0 - r + px, gy = y0 - r + py;
+        patch[i] = (gx >= 0 && gx < W && gy >= 0 && gy < H) ? src[(size_t)gy * W + gx] : T(0);
+    }
+    __syncthreads();
+    // pass 1, along rows: one thread per (patch row, 8 adjacent outputs).  Integer frames slide the box
+    // (add the entering value, subtract the leaving one: exact in integers); float frames re-sum every box.
+    for (int i = threadIdx.x; i < ph * (EQ_TW / 8); i += 256) {
+        const int py = i / (EQ_TW / 8), x8 = (i - py * (EQ_TW / 8)) * 8;
+        const T *p = patch + py * pw + x8;
+        S1 s = 0;
+        S2 s2 = 0;
+        for (int d = 0; d <= 2 * r; ++d) {
+            const S1 v = (S1)p[d];
+            s += v;
+            s2 += (S2)v * (S2)v;
+        }
+        h1[py * EQ_TW + x8] = s;
+        h2[py * EQ_TW + x8] = s2;
+        for (int k = 1; k < 8; ++k) {
+            if (sizeof(T) == 4) {
+                s = 0;
+                s2 = 0;
+                for (int d = 0; d <= 2 * r; ++d) {
+                    const S1 v = (S1)p[k + d];
+                    s += v;
+                    s2 += (S2)v * (S2)v;
+                }
+            } else {
+                const S1 a = (S1)p[k + 2 * r], b = (S1)p[k - 1];
+                s += a - b;
+                s2 += (S2)a * (S2)a - (S2)b * (S2)b;
+            }
+            h1[py * EQ_TW + x8 + k] = s;
+            h2[py * EQ_TW + x8 + k] = s2;
+        }
+    }
+    __syncthreads();
+    // pass 2, along columns: one thread per (column, 8 adjacent rows), same sliding rule; then normalise
+    {
+        const int x = threadIdx.x & (EQ_TW - 1), y8 = (threadIdx.x / EQ_TW) * 8;
+        const int gx = x0 + x;
+        S1 s = 0;
+        S2 s2 = 0;
+        for (int k = 0; k < 8; ++k) {
+            const int y = y8 + k, gy = y0 + y;
+            if (k == 0 || sizeof(T) == 4) {
+                s = 0;
+                s2 = 0;
+                for (int d = 0; d <= 2 * r; ++d) {
+                    s += h1[(y + d) * EQ_TW + x];
+                    s2 += h2[(y + d) * EQ_TW + x];
+                }
+            } else {
+                s += h1[(y + 2 * r) * EQ_TW + x] - h1[(y - 1) * EQ_TW + x];
+                s2 += h2[(y + 2 * r) * EQ_TW + x] - h2[(y - 1) * EQ_TW + x];
+            }
+            if (gx >= W || gy >= H) continue;
+            const int n = (min(gx + r, W - 1) - max(gx - r, 0) + 1) * (min(gy + r, H - 1) - max(gy - r, 0) + 1);
+            const T c = patch[(y + r) * pw + x + r];
+            float out;
+            if (sizeof(T) == 4) {                                          // float frames: fp64 moments
+                const double num = (double)n * (double)s2 - (double)s * (double)s;
+                out = num > 0.0 ? (float)(((double)c * n - (double)s) / sqrt(num)) : 0.f;
+            } else {                                                       // integer frames: exact numerators
+                const long long num = (long long)n * (long long)s2 - (long long)s * (long long)s;
+                const long long top = (long long)c * n - (long long)s;
+                out = num > 0 ? (float)top / sqrtf((float)num) : 0.f;
+            }
+            dst[(size_t)gy * pitch + gx] = out;
+        }
+    }
+}

@@ -6,6 +6,7 @@
 #include "../../include/optflow.h"
 #include "of_kernels.cuh"
 #include "of_solve.cuh"
+#include "of_equalise.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -85,6 +86,7 @@ struct of_context {
     int W, H, levels, R, iterations, window_type;
     int device;
     float eps_rel, max_step;
+    int eq_radius;                      // 0 = frames are converted as they are; > 0 = eq. 2 pre-filter of that radius
     Level lv[OF_MAX_LEVELS];
     float *pyr[N_PYR][OF_MAX_LEVELS];
     float *u[OF_MAX_LEVELS], *v[OF_MAX_LEVELS];
@@ -271,6 +273,17 @@ void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitc
 void run_convert(const of_context *c, int dtype, const void *a, const void *b, float *da, float *db, cudaStream_t st)
 {
     const Level &L = c->lv[0];
+    if (c->eq_radius > 0) {                                            // eq. 2 fused with the conversion
+        const int r = c->eq_radius;
+        dim3 grid((L.W + EQ_TW - 1) / EQ_TW, (L.H + EQ_TH - 1) / EQ_TH, b ? 2 : 1);
+        if (dtype == OF_DTYPE_U8)
+            k0_equalise<uint8_t><<<grid, 256, eq_smem_bytes(r, 1), st>>>((const uint8_t *)a, (const uint8_t *)b, da, db, L.W, L.H, L.pitch, r);
+        else if (dtype == OF_DTYPE_U16)
+            k0_equalise<uint16_t><<<grid, 256, eq_smem_bytes(r, 2), st>>>((const uint16_t *)a, (const uint16_t *)b, da, db, L.W, L.H, L.pitch, r);
+        else
+            k0_equalise<float><<<grid, 256, eq_smem_bytes(r, 4), st>>>((const float *)a, (const float *)b, da, db, L.W, L.H, L.pitch, r);
+        return;
+    }
     dim3 grid((L.W + 1023) / 1024, L.H, b ? 2 : 1);
     if (dtype == OF_DTYPE_U8)
         k0_convert<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)a, (const uint8_t *)b, da, db, L.W, L.H, L.pitch);
@@ -586,6 +599,21 @@ int of_set_conditioning(of_handle h, float eps_rel, float max_step_px)
     if (!(eps_rel >= 0.f) || !(max_step_px > 0.f)) return fail(OF_ERR_INVALID_ARG, "eps_rel must be >= 0 and max_step_px > 0");
     h->eps_rel = eps_rel;
     h->max_step = max_step_px;
+    drop_graphs(h);
+    return OF_OK;
+}
+
+int of_set_equalisation(of_handle h, int radius)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    if (radius < 0 || radius > OF_MAX_WINDOW_RADIUS) return fail(OF_ERR_INVALID_ARG, "equalisation radius must be in [0,%d]", OF_MAX_WINDOW_RADIUS);
+    if (radius > 0) {
+        CU_TRY(cudaSetDevice(h->device));
+        CU_TRY(cudaFuncSetAttribute(k0_equalise<uint8_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(OF_MAX_WINDOW_RADIUS, 1)));
+        CU_TRY(cudaFuncSetAttribute(k0_equalise<uint16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(OF_MAX_WINDOW_RADIUS, 2)));
+        CU_TRY(cudaFuncSetAttribute(k0_equalise<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(OF_MAX_WINDOW_RADIUS, 4)));
+    }
+    h->eq_radius = radius;
     drop_graphs(h);
     return OF_OK;
 }

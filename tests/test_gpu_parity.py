@@ -350,3 +350,47 @@ def test_errors_are_reported_not_thrown(B):
     assert B.lib().of_create(64, 64, 1, 4, 1, 7) in (None, 0)
     assert B.lib().of_compute(None, None, None, None, None, None) < 0
     B.lib().of_destroy(None)
+
+
+# ---------------------------------------------------------------------------- eq. 2 pre-filter (NEXT item f1)
+@pytest.mark.parametrize("dtype,W,H,r", [(np.uint8, 320, 256, 5), (np.uint16, 203, 131, 3), (np.float32, 130, 70, 5),
+                                         (np.uint8, 64, 40, 16)])
+def test_equalisation_kernel_matches_oracle(torch, B, oracle, dtype, W, H, r):
+    """of_set_equalisation: the level-0 plane is eq. 2 of the raw frame; flat
+    neighbourhoods give exactly 0 on both sides."""
+    rng = np.random.default_rng(W + H + r)
+    hi = {np.uint8: 256, np.uint16: 4096, np.float32: 256}[dtype]
+    I1 = rng.integers(0, hi, (H, W)).astype(dtype)
+    I2 = rng.integers(0, hi, (H, W)).astype(dtype)
+    I1[H // 4:H // 2, W // 4:W // 2] = 7                      # a flat patch larger than the box
+    ref1, ref2 = oracle.equalise(I1, r), oracle.equalise(I2, r)
+    R = min(3, (min(W, H) - 1) // 2)
+    with B.OpticalFlow(W, H, 1, R, 1, BOX) as of:
+        of.set_equalisation(r)
+        d1 = torch.from_numpy(I1.view(np.int16) if dtype == np.uint16 else I1).cuda()
+        d2 = torch.from_numpy(I2.view(np.int16) if dtype == np.uint16 else I2).cuda()
+        of.compute(d1, d2)
+        torch.cuda.synchronize()
+        g1, g2 = of.debug_plane(0, 0).cpu().numpy(), of.debug_plane(0, 1).cpu().numpy()
+    assert np.max(np.abs(g1 - ref1)) < 2e-5 and np.max(np.abs(g2 - ref2)) < 2e-5
+    assert np.array_equal(g1 == 0.0, ref1 == 0.0)
+
+
+def test_solve_with_equalisation_matches_oracle(torch, B, oracle):
+    """Whole path with the pre-filter on: unevenly lit config-3-like pair, parity at the usual bar."""
+    c = syn.config3(352, 288)
+    yy, xx = np.mgrid[0:288, 0:352]
+    lit = 0.6 + 0.4 * xx / 352.0
+    I2 = np.clip(np.rint(c.I2 * lit), 0, 255).astype(np.uint8)
+    ref = oracle.solve(oracle.equalise(c.I1, 5), oracle.equalise(I2, 5), 3, 6, 4, GAUSS)
+    with B.OpticalFlow(352, 288, 3, 6, 4, GAUSS) as of:
+        of.set_equalisation(5)
+        u, v = of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(I2).cuda())
+        m = of.validity()
+        torch.cuda.synchronize()
+        st = assert_parity(u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy(), ref, "equalised")
+        of.set_equalisation(0)
+        u0, v0 = of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(I2).cuda())
+        torch.cuda.synchronize()
+    ref0 = oracle.solve(c.I1, I2, 3, 6, 4, GAUSS)
+    assert_parity(u0.cpu().numpy(), v0.cpu().numpy(), None, ref0, "switched off again")

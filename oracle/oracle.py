@@ -164,3 +164,32 @@ def solve(I1, I2, levels, R, iterations, window_type, eps=EPS_REL, max_step=MAX_
     if return_levels:
         out["level_u"], out["level_v"] = lu, lv
     return out
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT item f3: recirculation-bubble surface, eq. 3.  The printed fraction is garbled
+# (D20); the text defines it: "the percentage of velocities below a given threshold T_v relative to the
+# total number of available velocity vectors", with T_v = 1/2 [min + max] of the longitudinal component
+# of the MEAN velocity field.  Plain NumPy, written out as the definition.
+# ---------------------------------------------------------------------------------------------
+def bubble_threshold(mean_vx, valid=None):
+    """T_v = (min + max) / 2 of the mean longitudinal velocity over the available vectors."""
+    m = np.asarray(mean_vx, dtype=np.float64)
+    if valid is not None:
+        m = m[np.asarray(valid).astype(bool)]
+    return 0.5 * (float(m.min()) + float(m.max()))
+
+
+def bubble_counts(vx, threshold, valid=None):
+    """(number of available vectors with v_x <= T_v, number of available vectors); S_bubble is their ratio."""
+    v = np.asarray(vx)
+    ok = np.ones(v.shape, dtype=bool) if valid is None else np.asarray(valid).astype(bool)
+    below = 0
+    total = 0
+    for row_v, row_ok in zip(v, ok):            # explicit count, row by row
+        for a, b in zip(row_v.tolist(), row_ok.tolist()):
+            if b:
+                total += 1
+                if a <= threshold:
+                    below += 1
+    return below, total

@@ -429,3 +429,31 @@ def test_flow_is_unchanged_by_equalisation_of_an_unevenly_lit_pair(oracle):
     err_raw = np.sqrt(np.mean((raw["u"][m] - d[0]) ** 2 + (raw["v"][m] - d[1]) ** 2))
     err_eq = np.sqrt(np.mean((eq["u"][m] - d[0]) ** 2 + (eq["v"][m] - d[1]) ** 2))
     assert err_eq < 0.5 * err_raw and err_eq < 0.05
+
+
+# ---------------------------------------------------------------------------- eq. 3 (NEXT item f3)
+def test_bubble_surface_definition_on_hand_worked_fields(oracle):
+    """eq. 3: share of available vectors with v_x <= T_v, T_v = mid-range of the mean field."""
+    mean = np.array([[-1.0, 0.0, 1.0], [2.0, 3.0, 7.0]])
+    assert oracle.bubble_threshold(mean) == 3.0                       # (min -1 + max 7) / 2
+    vx = np.array([[3.0, 3.5, -2.0], [2.9, 8.0, 3.0]])
+    assert oracle.bubble_counts(vx, 3.0) == (4, 6)                    # 3.0, -2.0, 2.9, 3.0 (<= is inclusive)
+    valid = np.array([[1, 1, 0], [1, 0, 1]], dtype=np.uint8)
+    assert oracle.bubble_counts(vx, 3.0, valid) == (3, 4)             # only available vectors count
+    assert oracle.bubble_threshold(mean, valid) == 3.0
+    # a linear profile v_x = x over [0, W-1]: T_v = (W-1)/2 and exactly the lower half (inclusive) is below
+    W = 11
+    lin = np.tile(np.arange(W, dtype=np.float64), (4, 1))
+    T = oracle.bubble_threshold(lin)
+    assert T == 5.0 and oracle.bubble_counts(lin, T) == (4 * 6, 4 * W)
+
+
+def test_bubble_surface_of_the_backward_step_like_truth_field(oracle):
+    """The config-3 ground-truth field has a -1 px recirculation region upstream of x = 0.7 W below the shear
+    layer: its bubble surface must be the area share of that region (cross-check of the definition with
+    a thresholded-area count done independently with NumPy)."""
+    c = syn.config3(320, 256)
+    T = oracle.bubble_threshold(c.truth_u)
+    below, total = oracle.bubble_counts(c.truth_u, T)
+    assert total == 320 * 256 and below == int(np.count_nonzero(c.truth_u <= T))
+    assert 0.15 < below / total < 0.45

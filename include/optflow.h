@@ -136,6 +136,21 @@ int of_run_solve(of_handle h, int repeat, void *stream);
  * written (0 if the hook was off), or a negative status. */
 int of_solve_timeline(of_handle h, int enable, int cta, unsigned long long *out_host, int max_entries);
 
+/* ---------------------------------------------------------------------------------------------
+ * Integral quantity of a field on the device (eq. 3: recirculation-bubble surface
+ * S_bubble = share of the available vectors with v_x <= T_v, T_v = (min + max)/2 of the mean field; "such
+ * an integral value could ... be used as an input in a feedback loop").  All pointers are device pointers
+ * to dense H x W arrays; valid_dev (may be NULL = every vector available) is a validity mask as returned
+ * by of_get_validity.  Asynchronous on `stream`; integer atomics only, so results are exact.
+ * ------------------------------------------------------------------------------------------- */
+/* sum_dev += field_dev (running sum for the mean field). */
+int of_field_accumulate(of_handle h, float *sum_dev, const float *field_dev, void *stream);
+/* out_dev[0] = min, out_dev[1] = max of field_dev over the available vectors (NaN ignored). */
+int of_field_minmax(of_handle h, const float *field_dev, const uint8_t *valid_dev, float *out_dev, void *stream);
+/* out_dev[0] = number of available vectors with vx <= threshold, out_dev[1] = number of available vectors. */
+int of_bubble_count(of_handle h, const float *vx_dev, const uint8_t *valid_dev, float threshold,
+                    unsigned long long *out_dev, void *stream);
+
 /* Stand-alone single steps (rows a2, a10 of the scope table), dense device buffers. */
 int of_pyramid_down(const float *src, int width, int height, float *dst, void *stream);
 int of_upsample_flow(const float *uc, const float *vc, int wc, int hc, float *u, float *v, int width,

@@ -39,6 +39,9 @@ SIGNATURES = {
     "of_get_debug_plane": (_i, [_vp, _i, _i, _vp, _vp]),
     "of_run_step": (_i, [_vp, _i, _i, _i, _vp]),
     "of_run_solve": (_i, [_vp, _i, _vp]),
+    "of_field_accumulate": (_i, [_vp, _vp, _vp, _vp]),
+    "of_field_minmax": (_i, [_vp, _vp, _vp, _vp, _vp]),
+    "of_bubble_count": (_i, [_vp, _vp, _vp, _c.c_float, _vp, _vp]),
     "of_pyramid_down": (_i, [_vp, _i, _i, _vp, _vp]),
     "of_upsample_flow": (_i, [_vp, _vp, _i, _i, _vp, _vp, _i, _i, _vp]),
     "of_stream_open": (_i, [_vp, _i, _i, _i]),
@@ -190,6 +193,23 @@ class OpticalFlow:
 
     def run_solve(self, repeat=1, stream=None):
         _check(lib().of_run_solve(self._h, repeat, _stream_ptr(stream)))
+
+    # -- integral quantity, eq. 3 -----------------------------------------------------------
+    def field_accumulate(self, total, field, stream=None):
+        _check(lib().of_field_accumulate(self._h, total.data_ptr(), field.data_ptr(), _stream_ptr(stream)))
+
+    def field_minmax(self, field, valid=None, stream=None):
+        out = self._torch.empty(2, dtype=self._torch.float32, device=field.device)
+        _check(lib().of_field_minmax(self._h, field.data_ptr(), valid.data_ptr() if valid is not None else None,
+                                     out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    def bubble_count(self, vx, threshold, valid=None, stream=None):
+        """Device tensor of two int64: (available vectors with vx <= threshold, available vectors)."""
+        out = self._torch.empty(2, dtype=self._torch.int64, device=vx.device)
+        _check(lib().of_bubble_count(self._h, vx.data_ptr(), valid.data_ptr() if valid is not None else None,
+                                     float(threshold), out.data_ptr(), _stream_ptr(stream)))
+        return out
 
     # -- frame pipeline -----------------------------------------------------------------------
     def stream_open(self, dtype, mode=OF_STREAM_CONSECUTIVE, result_on_host=True):

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liboptflow.so")
 SOURCES = ["optflow.cu"]
-DEPS = ["optflow.cu", "of_kernels.cuh", "of_common.cuh", "of_k2.cuh", "of_k3.cuh", "of_solve.cuh", "of_equalise.cuh", os.path.join("..", "..", "include", "optflow.h")]
+DEPS = ["optflow.cu", "of_kernels.cuh", "of_common.cuh", "of_k2.cuh", "of_k3.cuh", "of_solve.cuh", "of_equalise.cuh", "of_post.cuh", os.path.join("..", "..", "include", "optflow.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 

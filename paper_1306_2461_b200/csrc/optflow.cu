@@ -7,6 +7,7 @@
 #include "of_kernels.cuh"
 #include "of_solve.cuh"
 #include "of_equalise.cuh"
+#include "of_post.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -102,6 +103,7 @@ struct of_context {
     LevelDesc *d_lv;                    // device copies for the persistent solve kernel
     CUtensorMap *d_tm;
     unsigned *d_gbar;
+    unsigned *d_post;                   // scratch of the post-processing reductions (min/max words)
     unsigned long long *d_prof;         // timeline buffer of the persistent kernel (of_solve_timeline)
     bool prof_on;
     bool persistent;                    // whole solve in one cooperative launch (default) vs one launch per kernel
@@ -545,6 +547,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_lv, sizeof(LevelDesc) * levels);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_tm, sizeof(CUtensorMap) * levels);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_gbar, 256);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_post, 256);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_prof, sizeof(unsigned long long) * OF_TIMELINE_MAX * c->sms);
         if (rc == OF_OK) {
             LevelDesc hl[OF_MAX_LEVELS];
@@ -720,6 +723,38 @@ int of_run_solve(of_handle h, int repeat, void *stream)
         DISPATCH_R(h->R, e = launch_solve<R>(h, nullptr, 0, 1, h->S + 3 * h->plane, h->S + 4 * h->plane, st));
         if (e != cudaSuccess) return fail(OF_ERR_CUDA, "solve launch failed: %s", cudaGetErrorString(e));
     }
+    return OF_OK;
+}
+
+int of_field_accumulate(of_handle h, float *sum_dev, const float *field_dev, void *stream)
+{
+    if (!h || !sum_dev || !field_dev) return fail(OF_ERR_INVALID_ARG, "null argument");
+    const size_t n = (size_t)h->W * h->H;
+    kp_accumulate<<<2 * h->sms, 256, 0, (cudaStream_t)stream>>>(sum_dev, field_dev, n);
+    CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+int of_field_minmax(of_handle h, const float *field_dev, const uint8_t *valid_dev, float *out_dev, void *stream)
+{
+    if (!h || !field_dev || !out_dev) return fail(OF_ERR_INVALID_ARG, "null argument");
+    const size_t n = (size_t)h->W * h->H;
+    cudaStream_t st = (cudaStream_t)stream;
+    kp_minmax_init<<<1, 1, 0, st>>>(h->d_post);
+    kp_minmax<<<2 * h->sms, 256, 0, st>>>(field_dev, valid_dev, n, h->d_post);
+    kp_minmax_finish<<<1, 1, 0, st>>>(h->d_post, out_dev);
+    CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+int of_bubble_count(of_handle h, const float *vx_dev, const uint8_t *valid_dev, float threshold, unsigned long long *out_dev, void *stream)
+{
+    if (!h || !vx_dev || !out_dev) return fail(OF_ERR_INVALID_ARG, "null argument");
+    const size_t n = (size_t)h->W * h->H;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(cudaMemsetAsync(out_dev, 0, 2 * sizeof(unsigned long long), st));
+    kp_bubble_count<<<2 * h->sms, 256, 0, st>>>(vx_dev, valid_dev, n, threshold, out_dev);
+    CU_TRY(cudaGetLastError());
     return OF_OK;
 }
 

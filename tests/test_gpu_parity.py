@@ -394,3 +394,36 @@ def test_solve_with_equalisation_matches_oracle(torch, B, oracle):
         torch.cuda.synchronize()
     ref0 = oracle.solve(c.I1, I2, 3, 6, 4, GAUSS)
     assert_parity(u0.cpu().numpy(), v0.cpu().numpy(), None, ref0, "switched off again")
+
+
+# ---------------------------------------------------------------------------- eq. 3 bubble surface (NEXT item f3)
+def test_bubble_surface_counts_match_oracle_exactly(torch, B, oracle):
+    """Mean field over 3 solves -> T_v -> thresholded count on the device; integer results, compared exactly
+    with the oracle applied to the SAME fp32 fields (eq. 3)."""
+    W, H = 320, 256
+    with B.OpticalFlow(W, H, 2, 6, 3, BOX) as of:
+        total = torch.zeros((H, W), dtype=torch.float32, device="cuda")
+        fields = []
+        for k in range(3):
+            c = syn.config3(W, H, seed_offset=k)
+            u, v = of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda())
+            of.field_accumulate(total, u)
+            fields.append(u.clone())
+        m = of.validity()
+        mm = of.field_minmax(total, m)
+        torch.cuda.synchronize()
+        tot_h = fields[0].cpu().numpy().astype(np.float32)
+        for f in fields[1:]:
+            tot_h = tot_h + f.cpu().numpy()                       # same fp32 running sum, same order
+        assert np.array_equal(total.cpu().numpy(), tot_h)
+        mh = m.cpu().numpy()
+        lo, hi = float(mm[0]), float(mm[1])
+        assert lo == float(tot_h[mh != 0].min()) and hi == float(tot_h[mh != 0].max())
+        T = np.float32(0.5) * (np.float32(lo) + np.float32(hi)) / np.float32(3.0)      # mid-range of the MEAN field
+        assert abs(float(T) - oracle.bubble_threshold(tot_h.astype(np.float64) / 3.0, mh)) < 1e-5
+        cnt = of.bubble_count(fields[2], float(T), m)
+        cnt_all = of.bubble_count(fields[2], float(T))
+        torch.cuda.synchronize()
+        assert tuple(cnt.cpu().tolist()) == oracle.bubble_counts(fields[2].cpu().numpy(), float(T), mh)
+        assert tuple(cnt_all.cpu().tolist()) == oracle.bubble_counts(fields[2].cpu().numpy(), float(T))
+        assert 0 < cnt[0] < cnt[1] <= W * H

@@ -25,7 +25,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("OF_NVCC_DEFS", "").split() + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
         r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
         with open(os.path.join(HERE, "build.log"), "w") as f:
             f.write(" ".join(cmd) + "\n" + r.stdout)

@@ -2,10 +2,10 @@
 // scope table; BASELINE.json:5 "(3) Vertical-sum+solve kernel"; readings D11-D15 of DESIGN.md).
 //
 // Persistent, warp-specialised, one CTA per SM (sm_100a):
-//   * the image is cut into 64-column strips x 8-row blocks = "tasks"; task order is strip-major and
+//   * the image is cut into 64-column strips x K3_SEG-row blocks = "tasks"; task order is strip-major and
 //     every CTA owns an equal, contiguous run of tasks (grid = number of SMs, no tail wave);
 //   * the five horizontally summed planes are ONE 3-D tensor (x, y, field); a chunk = box of
-//     64 x 8 x 5 floats (10 KB) fetched by a single cp.async.bulk.tensor into a shared-memory ring;
+//     64 x K3_SEG x 5 floats (5 KB) fetched by a single cp.async.bulk.tensor into a shared-memory ring;
 //     rows above/below the image are zero-filled by the TMA unit, which IS the zero extension of the
 //     window (D12) -- no border code;
 //   * one PRODUCER warp walks the CTA's chunks in order: waits for the ring slot to be released
@@ -15,7 +15,7 @@
 //     sub-partitions), wait on the full barriers of their NC chunks, sum, release the chunks, solve.
 //     No __syncthreads after set-up.  Which warp runs a task does not change its arithmetic, so the
 //     result stays bit-reproducible (H8);
-//   * per lane (2 adjacent columns x 8 rows): (8+2R) LDS.64 per field feed 8*(2R+1) FFMA2 (packed
+//   * per lane (2 adjacent columns x K3_SEG rows): (K3_SEG+2R) LDS.64 per field feed K3_SEG*(2R+1) FFMA2 (packed
 //     fp32 pair FMA, scalar weight); then the damped 2x2 solve on the pair (D14), clamp (D15),
 //     update, validity byte.
 // Direct (2R+1)-tap sums, fixed order, no atomics on data: no cancellation (H2).
@@ -23,13 +23,20 @@
 #include "of_common.cuh"
 #include <cuda.h>
 
-#define K3_CHUNK_BYTES (64 * 8 * 5 * 4)
-#define K3_MAX_NW 11                                      // consumer warps (+1 producer warp)
-#define K3_RING 22                                        // chunks in the ring (220 KB)
+#ifndef K3_SEG
+#define K3_SEG 4                                          // rows per task = rows per TMA chunk (4: finer tasks, better
+                                                          // balance and shorter coarse-level passes than 8; measured)
+#endif
+#define K3_CHUNK_BYTES (64 * K3_SEG * 5 * 4)
+#ifndef K3_MAX_NW
+#define K3_MAX_NW 11
+#endif
+//                                     // consumer warps (+1 producer warp)
+#define K3_RING (176 / K3_SEG)                            // chunks in the ring (220 KB)
 
 template <int R> struct K3Geom {
-    static constexpr int NIN = 8 + 2 * R;                // input rows per task
-    static constexpr int NC = (NIN + 7) / 8;             // chunks spanned by one task
+    static constexpr int NIN = K3_SEG + 2 * R;           // input rows per task
+    static constexpr int NC = (NIN + K3_SEG - 1) / K3_SEG;   // chunks spanned by one task
     static constexpr int SMEM = K3_RING * K3_CHUNK_BYTES + 2 * K3_RING * 8 + 16;
 };
 
@@ -162,14 +169,14 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
                 const int ntask = min(nrb - rb0, t_end - t);
                 const int total = ntask + NC - 1;
                 const int gbase = (int)gc0 + (t - t_begin) + (s - s_first) * (NC - 1);
-                const int x0 = 64 * s, yc0 = 8 * rb0 - R;               // chunk c holds rows yc0+8c .. +7
+                const int x0 = 64 * s, yc0 = K3_SEG * rb0 - R;          // chunk c holds rows yc0 + K3_SEG*c ...
                 for (int c = 0; c < total; ++c) {
                     const int gc = gbase + c, slot = gc % K3_RING, use = gc / K3_RING;
                     if (use > 0) mbar_wait(empty0 + 8 * slot, (use - 1) & 1);
                     const int readers = min(ntask - 1, c) - max(0, c - NC + 1) + 1;
                     if (readers < NC) mbar_arrive(empty0 + 8 * slot, NC - readers);   // stand-ins for tasks that do not exist
                     mbar_expect_tx(full0 + 8 * slot, K3_CHUNK_BYTES);
-                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + 8 * c, 0, full0 + 8 * slot);
+                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + K3_SEG * c, 0, full0 + 8 * slot);
                 }
                 t += ntask;
             }
@@ -185,14 +192,14 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         if (i >= t_end - t_begin) break;
         const int gt = t_begin + i, s = gt / nrb, rb = gt - s * nrb;
         const int gbase = (int)gc0 + i + (s - s_first) * (NC - 1);
-        const int gx = 64 * s + 2 * lane, gy0 = 8 * rb;
+        const int gx = 64 * s + 2 * lane, gy0 = K3_SEG * rb;
         const bool active = gx < W;
         // this lane's field values, issued before the waits (rows past the image re-read the last row)
-        const int nrows = min(8, H - gy0);
+        const int nrows = min(K3_SEG, H - gy0);
         const float *ui = p.u_in + (size_t)gy0 * pitch + gx, *vi = p.v_in + (size_t)gy0 * pitch + gx;
-        float2 uu[8], vv[8];
+        float2 uu[K3_SEG], vv[K3_SEG];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < K3_SEG; ++j) {
             const int jj = min(j, nrows - 1) * pitch;
             uu[j] = active ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
             vv[j] = active ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
@@ -207,20 +214,20 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             fb[k] = full0 + 8 * slot;
             fpar[k] = (gc / K3_RING) & 1;
         }
-        float2 acc[5][8];
+        float2 acc[5][K3_SEG];
 #pragma unroll
         for (int f = 0; f < 5; ++f)
 #pragma unroll
-            for (int j = 0; j < 8; ++j) acc[f][j] = make_float2(0.f, 0.f);
+            for (int j = 0; j < K3_SEG; ++j) acc[f][j] = make_float2(0.f, 0.f);
         if (!(p.dbg & 2))
 #pragma unroll
         for (int r = 0; r < G::NIN; ++r) {
-            if ((r & 7) == 0 && !(p.dbg & 1)) mbar_wait(fb[r >> 3], fpar[r >> 3]);   // chunk by chunk, as the TMA delivers them
+            if ((r % K3_SEG) == 0 && !(p.dbg & 1)) mbar_wait(fb[r / K3_SEG], fpar[r / K3_SEG]);   // chunk by chunk, as the TMA delivers them
 #pragma unroll
             for (int f = 0; f < 5; ++f) {
-                const float2 val = *reinterpret_cast<const float2 *>(cb[r >> 3] + f * 2048 + (r & 7) * 256);
+                const float2 val = *reinterpret_cast<const float2 *>(cb[r / K3_SEG] + f * (K3_SEG * 256) + (r % K3_SEG) * 256);
 #pragma unroll
-                for (int j = 0; j < 8; ++j)
+                for (int j = 0; j < K3_SEG; ++j)
                     if (r - j >= 0 && r - j <= 2 * R) acc[f][j] = fma2s(p.ww.w[r - j], val, acc[f][j]);
             }
         }
@@ -234,9 +241,9 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         const bool pair_ok = gx + 1 < W;
         const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
         float *uo = p.u_out + (size_t)gy0 * p.out_pitch + gx, *vo = p.v_out + (size_t)gy0 * p.out_pitch + gx;
-        float2 trs[8], dets[8];
+        float2 trs[K3_SEG], dets[K3_SEG];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < K3_SEG; ++j) {
             float2 du, dv;
             k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, trs[j], dets[j]);
             const float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
@@ -254,7 +261,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             uint8_t *m = p.valid + (size_t)gy0 * W + gx;
             float *d = p.det + (size_t)gy0 * pitch + gx;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
+            for (int j = 0; j < K3_SEG; ++j) {
                 if (j < nrows) {
                     m[j * W] = trs[j].x > 0.f ? 1 : 0;
                     d[j * pitch] = dets[j].x;

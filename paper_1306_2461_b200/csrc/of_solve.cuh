@@ -21,7 +21,10 @@
 #include "of_k3.cuh"
 
 #define SOLVE_TIMELINE_MAX 4096
-#define SOLVE_WARPS 12                       // 11 K3 consumers + 1 producer; all 12 work in the K2 pass
+#ifndef SOLVE_WARPS
+#define SOLVE_WARPS 12
+#endif
+//                      // 11 K3 consumers + 1 producer; all 12 work in the K2 pass
 
 struct LevelDesc {
     const float *pyr[2];                     // pyramid slots (I1 / I2 chosen per job)

@@ -177,7 +177,7 @@ template <int R> K2Plan plan_k2(int W, int H, int sms)
 template <int R> K3Plan plan_k3(int W, int H, int sms)
 {
     K3Plan p = {};
-    p.nrb = (H + 7) / 8;
+    p.nrb = (H + K3_SEG - 1) / K3_SEG;
     p.ntasks = ((W + 63) / 64) * p.nrb;
     p.grid = sms;
     p.warps = SOLVE_WARPS - 1;                                  // consumer warps; one producer warp is added at launch
@@ -240,7 +240,7 @@ int encode_tensor_maps(of_context *c)
         const Level &L = c->lv[l];
         cuuint64_t dims[3] = {(cuuint64_t)L.pitch, (cuuint64_t)L.H, 5};
         cuuint64_t strides[2] = {(cuuint64_t)L.pitch * sizeof(float), (cuuint64_t)c->plane * sizeof(float)};
-        cuuint32_t box[3] = {64, 8, 5};
+        cuuint32_t box[3] = {64, K3_SEG, 5};
         cuuint32_t estr[3] = {1, 1, 1};
         CUresult r = ((encode_fn)fn)(&c->tmS[l], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, c->S, dims, strides, box, estr,
                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,

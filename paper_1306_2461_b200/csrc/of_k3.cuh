@@ -8,7 +8,7 @@
 //     64 x K3_SEG x 5 floats (5 KB) fetched by a single cp.async.bulk.tensor into a shared-memory ring;
 //     rows above/below the image are zero-filled by the TMA unit, which IS the zero extension of the
 //     window (D12) -- no border code;
-//   * one PRODUCER warp walks the CTA's chunks in order: waits for the ring slot to be released
+//   * one PRODUCER warp (it joins the consumers when it has issued its last chunk) walks the CTA's chunks in order: waits for the ring slot to be released
 //     (empty mbarrier, NC arrivals = the NC tasks that read a chunk), arms the full mbarrier with
 //     expect_tx and issues the TMA;
 //   * up to 8 CONSUMER warps pull tasks from a shared-memory counter (balances the four SM
@@ -181,7 +181,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
                 t += ntask;
             }
         }
-        return;
+        __syncwarp();                                   // production done (or nothing to produce): join the consumers
     }
 
     // ========================= consumers

@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(256) k0_convert(const T *__restrict__ srcA, co
 // CTA = 32x8 outputs; source patch (2*32+3) x (2*8+3) staged in shared memory with clamped indices,
 // rows filtered first, then columns (same order as the definition).
 // ------------------------------------------------------------------------------------------------
-#define K1_TW 32
+#define K1_TW 32                                   // (the index arithmetic below relies on K1_TW == 32)
 #define K1_TH 8
 __global__ void __launch_bounds__(256) k1_pyramid_down(const float *__restrict__ srcA, const float *__restrict__ srcB,
                                                        float *__restrict__ dstA, float *__restrict__ dstB,
@@ -65,14 +65,18 @@ __global__ void __launch_bounds__(256) k1_pyramid_down(const float *__restrict__
     __shared__ float T[2 * K1_TH + 3][K1_TW + 1];
     const int X0 = blockIdx.x * K1_TW, Y0 = blockIdx.y * K1_TH;
     const int sx0 = 2 * X0 - 2, sy0 = 2 * Y0 - 2;
-    for (int i = threadIdx.x; i < (2 * K1_TH + 3) * (2 * K1_TW + 3); i += 256) {
-        int r = i / (2 * K1_TW + 3), c = i - r * (2 * K1_TW + 3);
-        int sy = clampi(sy0 + r, 0, H - 1), sx = clampi(sx0 + c, 0, W - 1);
-        patch[r][c] = __ldg(src + (size_t)sy * spitch + sx);
+    {   // 2-D walk over the patch (no division): thread (tx, ty) loads columns tx, tx+32, tx+64 of rows ty, ty+8, ty+16
+        const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+        for (int r = ty; r < 2 * K1_TH + 3; r += 8) {
+            const float *row = src + (size_t)clampi(sy0 + r, 0, H - 1) * spitch;
+#pragma unroll
+            for (int c = tx; c < 2 * K1_TW + 3; c += 32) patch[r][c] = __ldg(row + clampi(sx0 + c, 0, W - 1));
+        }
     }
     __syncthreads();
     for (int i = threadIdx.x; i < (2 * K1_TH + 3) * K1_TW; i += 256) {
-        int r = i / K1_TW, X = i - r * K1_TW;
+        int r = i >> 5, X = i & 31;
         const float *p = &patch[r][2 * X];
         float s = 0.0625f * p[0];
         s = fmaf(0.25f, p[1], s);

@@ -96,27 +96,32 @@ __device__ __forceinline__ void prof_stamp(const SolveArgs &a, int &idx)
 // Flow hand-down (row a10, D6): u_l = 2*bilinear(u_{l+1}; x/2, y/2), grid-stride over the fine level.
 __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDesc &C, int gtid, int nthreads)
 {
-    const int W = F.W, H = F.H, Wc = C.W, Hc = C.H, cp = C.pitch, hw = (W + 1) >> 1;
-    for (int i = gtid; i < hw * H; i += nthreads) {              // two adjacent fine pixels per thread
-        const int y = i / hw, x = 2 * (i - y * hw);
-        const int x0 = x >> 1, x1 = min(x0 + 1, Wc - 1), y0 = y >> 1, y1 = min(y0 + 1, Hc - 1);
-        const float fy = (y & 1) * 0.5f;
-        const float a00 = __ldcg(C.u + y0 * cp + x0), a01 = __ldcg(C.u + y0 * cp + x1);
-        const float a10 = __ldcg(C.u + y1 * cp + x0), a11 = __ldcg(C.u + y1 * cp + x1);
-        const float b00 = __ldcg(C.v + y0 * cp + x0), b01 = __ldcg(C.v + y0 * cp + x1);
-        const float b10 = __ldcg(C.v + y1 * cp + x0), b11 = __ldcg(C.v + y1 * cp + x1);
-        // even x: fx = 0; odd x (= x+1): fx = 1/2
-        const float ue = 2.0f * ((1.0f - fy) * a00 + fy * a10);
-        const float ve = 2.0f * ((1.0f - fy) * b00 + fy * b10);
-        const float uo = 2.0f * ((1.0f - fy) * (0.5f * a00 + 0.5f * a01) + fy * (0.5f * a10 + 0.5f * a11));
-        const float vo = 2.0f * ((1.0f - fy) * (0.5f * b00 + 0.5f * b01) + fy * (0.5f * b10 + 0.5f * b11));
+    const int W = F.W, H = F.H, Wc = C.W, Hc = C.H, cp = C.pitch, qw = (W + 3) >> 2;
+    for (int i = gtid; i < qw * H; i += nthreads) {              // four adjacent fine pixels per thread
+        const int y = i / qw, x = 4 * (i - y * qw);
+        const int x0 = x >> 1, x1 = min(x0 + 1, Wc - 1), x2 = min(x0 + 2, Wc - 1), y0 = y >> 1, y1 = min(y0 + 1, Hc - 1);
+        const float fy = (y & 1) * 0.5f, gy = 1.0f - fy;
+        const float *ur0 = C.u + y0 * cp, *ur1 = C.u + y1 * cp, *vr0 = C.v + y0 * cp, *vr1 = C.v + y1 * cp;
+        const float a00 = __ldcg(ur0 + x0), a01 = __ldcg(ur0 + x1), a02 = __ldcg(ur0 + x2);
+        const float a10 = __ldcg(ur1 + x0), a11 = __ldcg(ur1 + x1), a12 = __ldcg(ur1 + x2);
+        const float b00 = __ldcg(vr0 + x0), b01 = __ldcg(vr0 + x1), b02 = __ldcg(vr0 + x2);
+        const float b10 = __ldcg(vr1 + x0), b11 = __ldcg(vr1 + x1), b12 = __ldcg(vr1 + x2);
+        // even fine x: fx = 0; odd fine x: fx = 1/2 (same expression tree as k4_upsample_flow)
+        float uo[4], vo[4];
+        uo[0] = 2.0f * (gy * (1.0f * a00 + 0.0f * a01) + fy * (1.0f * a10 + 0.0f * a11));
+        uo[1] = 2.0f * (gy * (0.5f * a00 + 0.5f * a01) + fy * (0.5f * a10 + 0.5f * a11));
+        uo[2] = 2.0f * (gy * (1.0f * a01 + 0.0f * a02) + fy * (1.0f * a11 + 0.0f * a12));
+        uo[3] = 2.0f * (gy * (0.5f * a01 + 0.5f * a02) + fy * (0.5f * a11 + 0.5f * a12));
+        vo[0] = 2.0f * (gy * (1.0f * b00 + 0.0f * b01) + fy * (1.0f * b10 + 0.0f * b11));
+        vo[1] = 2.0f * (gy * (0.5f * b00 + 0.5f * b01) + fy * (0.5f * b10 + 0.5f * b11));
+        vo[2] = 2.0f * (gy * (1.0f * b01 + 0.0f * b02) + fy * (1.0f * b11 + 0.0f * b12));
+        vo[3] = 2.0f * (gy * (0.5f * b01 + 0.5f * b02) + fy * (0.5f * b11 + 0.5f * b12));
         float *pu = F.u + y * F.pitch + x, *pv = F.v + y * F.pitch + x;
-        if (x + 1 < W) {
-            *reinterpret_cast<float2 *>(pu) = make_float2(ue, uo);
-            *reinterpret_cast<float2 *>(pv) = make_float2(ve, vo);
+        if (x + 3 < W) {
+            *reinterpret_cast<float4 *>(pu) = make_float4(uo[0], uo[1], uo[2], uo[3]);
+            *reinterpret_cast<float4 *>(pv) = make_float4(vo[0], vo[1], vo[2], vo[3]);
         } else {
-            *pu = ue;
-            *pv = ve;
+            for (int k = 0; x + k < W; ++k) { pu[k] = uo[k]; pv[k] = vo[k]; }
         }
     }
 }

@@ -20,9 +20,8 @@
 #include "of_common.cuh"
 
 #ifndef K2_MAX_WARPS
-#define K2_MAX_WARPS 12
+#define K2_MAX_WARPS 12                            // warps per CTA (independent of each other); runtime blockDim
 #endif
-//                           // warps per CTA (independent of each other); runtime blockDim
 
 template <int R> struct K2Geom {
     static constexpr int RL = (R + 3) / 4 * 4;     // left/right halo rounded up: aligned vector loads

@@ -8,10 +8,10 @@
 //     64 x K3_SEG x 5 floats (5 KB) fetched by a single cp.async.bulk.tensor into a shared-memory ring;
 //     rows above/below the image are zero-filled by the TMA unit, which IS the zero extension of the
 //     window (D12) -- no border code;
-//   * one PRODUCER warp (it joins the consumers when it has issued its last chunk) walks the CTA's chunks in order: waits for the ring slot to be released
+//   * one PRODUCER warp walks the CTA's chunks in order: waits for the ring slot to be released
 //     (empty mbarrier, NC arrivals = the NC tasks that read a chunk), arms the full mbarrier with
-//     expect_tx and issues the TMA;
-//   * up to 8 CONSUMER warps pull tasks from a shared-memory counter (balances the four SM
+//     expect_tx and issues the TMA; when its last chunk is issued it joins the consumers;
+//   * the CONSUMER warps (K3_MAX_NW = 11) pull tasks from a shared-memory counter (balances the four SM
 //     sub-partitions), wait on the full barriers of their NC chunks, sum, release the chunks, solve.
 //     No __syncthreads after set-up.  Which warp runs a task does not change its arithmetic, so the
 //     result stays bit-reproducible (H8);
@@ -29,9 +29,8 @@
 #endif
 #define K3_CHUNK_BYTES (64 * K3_SEG * 5 * 4)
 #ifndef K3_MAX_NW
-#define K3_MAX_NW 11
+#define K3_MAX_NW 11                                      // consumer warps (+1 producer warp)
 #endif
-//                                     // consumer warps (+1 producer warp)
 #define K3_RING (176 / K3_SEG)                            // chunks in the ring (220 KB)
 
 template <int R> struct K3Geom {
@@ -237,7 +236,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             for (int k = 0; k < NC; ++k) mbar_arrive(eb[k], 1);
         }
         if (!active || (p.dbg & 4)) continue;
-        // ---- solve + update for 8 rows x 2 columns
+        // ---- solve + update for K3_SEG rows x 2 columns
         const bool pair_ok = gx + 1 < W;
         const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
         float *uo = p.u_out + (size_t)gy0 * p.out_pitch + gx, *vo = p.v_out + (size_t)gy0 * p.out_pitch + gx;

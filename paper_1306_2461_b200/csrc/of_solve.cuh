@@ -22,9 +22,8 @@
 
 #define SOLVE_TIMELINE_MAX 4096
 #ifndef SOLVE_WARPS
-#define SOLVE_WARPS 12
+#define SOLVE_WARPS 12                       // 11 K3 consumers + 1 producer; all 12 work in the K2 pass
 #endif
-//                      // 11 K3 consumers + 1 producer; all 12 work in the K2 pass
 
 struct LevelDesc {
     const float *pyr[2];                     // pyramid slots (I1 / I2 chosen per job)

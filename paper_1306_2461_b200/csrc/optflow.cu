@@ -173,7 +173,7 @@ template <int R> K2Plan plan_k2(int W, int H, int sms)
     return best;
 }
 
-// K3: tasks of 64 columns x 8 rows, equal contiguous share per CTA, one CTA per SM, NW tasks per step.
+// K3: tasks of 64 columns x K3_SEG rows, equal contiguous share per CTA, one CTA per SM.
 template <int R> K3Plan plan_k3(int W, int H, int sms)
 {
     K3Plan p = {};

@@ -13,7 +13,7 @@
 //   * u, v are rewritten by the K3 pass and read by the next K2 pass on other SMs: both sides use
 //     L2-only accesses (ld.global.cg) and the barrier carries __threadfence + acquire/release.
 //   * the five planes are written with ordinary stores and read by the TMA unit (async proxy): the
-//     producer lane issues fence.proxy.async after the barrier and before its first TMA.
+//     producer lane issues fence.proxy.async.global after the barrier and before its first TMA.
 //   * shared memory is a union of the K2 warp slices and the K3 ring: fence.proxy.async.shared::cta
 //     after the K2 pass orders its generic-proxy stores before the TMA writes of the K3 pass.
 #pragma once
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             const bool last = (l == 0 && it == a.iterations - 1);
             K3Params p3 = {L.u, L.v, last ? a.u_out : L.u, last ? a.v_out : L.v, last ? a.valid : nullptr, last ? a.det : nullptr,
                            L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, a.dbg};
-            if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async;" ::: "memory");
+            if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async.global;" ::: "memory");
             k3_phase<R>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
             gc0 += k3_chunks;
             __syncthreads();

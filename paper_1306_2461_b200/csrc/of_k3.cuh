@@ -31,7 +31,9 @@
 #ifndef K3_MAX_NW
 #define K3_MAX_NW 11                                      // consumer warps (+1 producer warp)
 #endif
+#ifndef K3_RING
 #define K3_RING (176 / K3_SEG)                            // chunks in the ring (220 KB)
+#endif
 
 template <int R> struct K3Geom {
     static constexpr int NIN = K3_SEG + 2 * R;           // input rows per task

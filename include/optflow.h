@@ -121,7 +121,7 @@ int of_get_debug_plane(of_handle h, int level, int which, float *out_dev, void *
  *   in place on the internal field). */
 int of_run_step(of_handle h, int level, int which, int repeat, void *stream);
 
-/* Launch ONLY the persistent solve kernel (plus the two memsets of the coarsest field), `repeat` times,
+/* Launch ONLY the persistent solve kernel, `repeat` times,
  * on the pyramids left by the last of_compute*; the level-0 result is discarded into scratch.  For
  * timing the dominant kernel with CUDA events and for ncu. */
 int of_run_solve(of_handle h, int repeat, void *stream);

@@ -40,6 +40,8 @@ struct K2Params {
     int nseg, nrp;                                 // lane layout of a warp tile
     int tiles_y, ntiles;                           // tile t -> (tx = t / tiles_y, ty = t % tiles_y)
     WinWeights ww;
+    int zero_uv;                                   // 1 = the field is identically zero (first iteration at the coarsest level,
+                                                   // PAPER.md:61 "initial guess of zero displacement"): u, v are not read
     int dbg;                                       // profiling switches (0 in production): 1 = no product phase, 2 = no sum phase, 32 = no plane stores
 };
 
@@ -72,11 +74,15 @@ __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
     in.c0 = __ldg(reinterpret_cast<const float2 *>(c));
     in.c1 = __ldg(reinterpret_cast<const float2 *>(c1p));
     in.c2 = __ldg(reinterpret_cast<const float2 *>(ptr_at(c, d2)));
-    const float *pu = ptr_at(p.u, i0), *pv = ptr_at(p.v, i0);
-    in.u0 = __ldcg(reinterpret_cast<const float2 *>(pu));
-    in.u1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pu, d1)));
-    in.v0 = __ldcg(reinterpret_cast<const float2 *>(pv));
-    in.v1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pv, d1)));
+    if (p.zero_uv) {
+        in.u0 = in.u1 = in.v0 = in.v1 = make_float2(0.f, 0.f);
+    } else {
+        const float *pu = ptr_at(p.u, i0), *pv = ptr_at(p.v, i0);
+        in.u0 = __ldcg(reinterpret_cast<const float2 *>(pu));
+        in.u1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pu, d1)));
+        in.v0 = __ldcg(reinterpret_cast<const float2 *>(pv));
+        in.v1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pv, d1)));
+    }
     // left / right neighbours with clamp-to-edge: x-1 -> x at the left border, x+2 -> W-1 at the right
     const int ol = x > 0 ? -1 : 0, orr = x + 2 < W ? 2 : (x + 1 < W ? 1 : 0);
     in.l0 = __ldg(ptr_at(c, ol));

@@ -52,6 +52,7 @@ struct K3Params {
     int nrb, ntasks;                 // row blocks per strip; ntasks = nstrips * nrb
     WinWeights ww;
     SolveParams sp;
+    int zero_uv;                     // 1 = the incoming field is identically zero and is not read (see of_k2.cuh)
     int dbg;                         // profiling switches (0 in production): 1 = no TMA/no waits, 2 = no window sum, 4 = no solve
 };
 
@@ -202,8 +203,8 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
 #pragma unroll
         for (int j = 0; j < K3_SEG; ++j) {
             const int jj = min(j, nrows - 1) * pitch;
-            uu[j] = active ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
-            vv[j] = active ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
+            uu[j] = (active && !p.zero_uv) ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
+            vv[j] = (active && !p.zero_uv) ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
         }
         const unsigned char *cb[NC];
         uint32_t eb[NC], fb[NC], fpar[NC];

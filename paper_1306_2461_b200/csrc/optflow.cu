@@ -192,21 +192,21 @@ template <int R> void plan_level(of_context *c, int l)
 }
 
 template <int R>
-void launch_k2(const of_context *c, int l, const float *I1, const float *I2, cudaStream_t st)
+void launch_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
 {
     const Level &L = c->lv[l];
     const K2Plan &P = c->k2[l];
-    K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, P.ntiles, c->ww, c->dbg};
+    K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, P.ntiles, c->ww, zero_uv ? 1 : 0, c->dbg};
     k2_products_hsum<R><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
 }
 
 template <int R>
-void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, cudaStream_t st)
+void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st)
 {
     const Level &L = c->lv[l];
     const K3Plan &P = c->k3[l];
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
-                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, c->dbg};
+                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg};
     k3_vsum_solve<R><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
@@ -263,13 +263,13 @@ int encode_tensor_maps(of_context *c)
     default: break;                                                                                \
     }
 
-void run_k2(const of_context *c, int l, const float *I1, const float *I2, cudaStream_t st)
+void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
 {
-    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, st));
+    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, zero_uv, st));
 }
-void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, cudaStream_t st)
+void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st)
 {
-    DISPATCH_R(c->R, launch_k3<R>(c, l, u_out, v_out, out_pitch, last, st));
+    DISPATCH_R(c->R, launch_k3<R>(c, l, u_out, v_out, out_pitch, last, zero_uv, st));
 }
 
 void run_convert(const of_context *c, int dtype, const void *a, const void *b, float *da, float *db, cudaStream_t st)
@@ -336,10 +336,7 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
             ++n;
         }
     }
-    const int top = c->levels - 1;
-    cudaMemsetAsync(c->u[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
-    cudaMemsetAsync(c->v[top], 0, sizeof(float) * (size_t)c->lv[top].pitch * c->lv[top].H, st);
-    note_launch(c, "memset", top);
+    const int top = c->levels - 1;     // (no memset of the coarsest field: its first iteration takes u = v = 0 without reading it)
     if (c->persistent) {
         cudaError_t e = cudaSuccess;
         DISPATCH_R(c->R, e = launch_solve<R>(c, nullptr, j.s1, j.s2, j.u_out, j.v_out, st));
@@ -350,11 +347,12 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
     for (int l = top; l >= 0; --l) {
         if (l < top) { run_upsample(c, l, st); note_launch(c, "upsample", l); ++n; }
         for (int it = 0; it < c->iterations; ++it) {
-            run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], st);
+            const bool zero_uv = (l == top && it == 0);
+            run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], zero_uv, st);
             note_launch(c, "products+hsum", l);
             const bool last = (l == 0 && it == c->iterations - 1);
-            if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, st);
-            else run_k3(c, l, c->u[l], c->v[l], c->lv[l].pitch, false, st);
+            if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, zero_uv, st);
+            else run_k3(c, l, c->u[l], c->v[l], c->lv[l].pitch, false, zero_uv, st);
             note_launch(c, "vsum+solve", l);
             n += 2;
         }
@@ -700,8 +698,8 @@ int of_run_step(of_handle h, int level, int which, int repeat, void *stream)
     if (!h || level < 0 || level >= h->levels || which < 0 || which > 1 || repeat < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
     CU_TRY(cudaSetDevice(h->device));
     for (int i = 0; i < repeat; ++i) {
-        if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], (cudaStream_t)stream);
-        else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, (cudaStream_t)stream);
+        if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], false, (cudaStream_t)stream);
+        else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, false, (cudaStream_t)stream);
     }
     CU_TRY(cudaGetLastError());
     return OF_OK;
@@ -713,11 +711,7 @@ int of_run_solve(of_handle h, int repeat, void *stream)
     if (!h->persistent) return fail(OF_ERR_STATE, "persistent mode is off");
     CU_TRY(cudaSetDevice(h->device));
     cudaStream_t st = (cudaStream_t)stream;
-    const int top = h->levels - 1;
-    const size_t top_bytes = sizeof(float) * (size_t)h->lv[top].pitch * h->lv[top].H;
     for (int i = 0; i < repeat; ++i) {
-        CU_TRY(cudaMemsetAsync(h->u[top], 0, top_bytes, st));
-        CU_TRY(cudaMemsetAsync(h->v[top], 0, top_bytes, st));
         cudaError_t e = cudaSuccess;
         // the level-0 result goes to the handle's own scratch (first two planes of S are free after the solve)
         DISPATCH_R(h->R, e = launch_solve<R>(h, nullptr, 0, 1, h->S + 3 * h->plane, h->S + 4 * h->plane, st));

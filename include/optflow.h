@@ -105,8 +105,8 @@ int of_get_validity(of_handle h, uint8_t *mask_dev, void *stream);
 int of_level_size(of_handle h, int level, int *width, int *height);
 
 /* Number of kernel launches (graph kernel nodes included) enqueued by the last of_compute* call:
- * persistent mode 1 (convert) + levels-1 (pyramid) + 1 (solve); otherwise + levels-1 hand-downs and
- * 2*levels*iterations iteration kernels instead of the solve. */
+ * persistent mode max(levels-1, 1) (frame conversion fused into the first pyramid step) + 1 (solve); otherwise
+ * + levels-1 hand-downs and 2*levels*iterations iteration kernels instead of the solve. */
 int of_last_launch_count(of_handle h);
 
 /* Test / profiling hooks.  State is that left by the last of_compute* on this handle.

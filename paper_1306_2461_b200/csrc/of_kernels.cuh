@@ -55,23 +55,37 @@ __global__ void __launch_bounds__(256) k0_convert(const T *__restrict__ srcA, co
 // ------------------------------------------------------------------------------------------------
 #define K1_TW 32                                   // (the index arithmetic below relies on K1_TW == 32)
 #define K1_TH 8
-__global__ void __launch_bounds__(256) k1_pyramid_down(const float *__restrict__ srcA, const float *__restrict__ srcB,
+// T = float: level l -> l+1 of an fp32 pyramid.  T = uint8_t / uint16_t / float with cvtA/cvtB != NULL: the first
+// step of a pair, fused with the frame conversion (row a1): the source is the raw dense frame (pitch == W) and
+// every CTA also writes the fp32 level-0 plane for the core of its patch (each source pixel belongs to exactly
+// one core), so the raw frame is read once and level 0 is never re-read by a separate conversion kernel.
+template <typename T>
+__global__ void __launch_bounds__(256) k1_pyramid_down(const T *__restrict__ srcA, const T *__restrict__ srcB,
                                                        float *__restrict__ dstA, float *__restrict__ dstB,
-                                                       int W, int H, int spitch, int Wd, int Hd, int dpitch)
+                                                       int W, int H, int spitch, int Wd, int Hd, int dpitch,
+                                                       float *__restrict__ cvtA, float *__restrict__ cvtB, int cpitch)
 {
-    const float *__restrict__ src = blockIdx.z ? srcB : srcA;
+    const T *__restrict__ src = blockIdx.z ? srcB : srcA;
     float *__restrict__ dst = blockIdx.z ? dstB : dstA;
+    float *__restrict__ cvt = blockIdx.z ? cvtB : cvtA;
     __shared__ float patch[2 * K1_TH + 3][2 * K1_TW + 4];
-    __shared__ float T[2 * K1_TH + 3][K1_TW + 1];
+    __shared__ float T_[2 * K1_TH + 3][K1_TW + 1];
     const int X0 = blockIdx.x * K1_TW, Y0 = blockIdx.y * K1_TH;
     const int sx0 = 2 * X0 - 2, sy0 = 2 * Y0 - 2;
     {   // 2-D walk over the patch (no division): thread (tx, ty) loads columns tx, tx+32, tx+64 of rows ty, ty+8, ty+16
         const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
 #pragma unroll
         for (int r = ty; r < 2 * K1_TH + 3; r += 8) {
-            const float *row = src + (size_t)clampi(sy0 + r, 0, H - 1) * spitch;
+            const int sy = sy0 + r;
+            const T *row = src + (size_t)clampi(sy, 0, H - 1) * spitch;
 #pragma unroll
-            for (int c = tx; c < 2 * K1_TW + 3; c += 32) patch[r][c] = __ldg(row + clampi(sx0 + c, 0, W - 1));
+            for (int c = tx; c < 2 * K1_TW + 3; c += 32) {
+                const int sx = sx0 + c;
+                const float val = (float)__ldg(row + clampi(sx, 0, W - 1));
+                patch[r][c] = val;
+                if (cvt != nullptr && r >= 2 && r < 2 * K1_TH + 2 && c >= 2 && c < 2 * K1_TW + 2 && sx < W && sy < H)
+                    cvt[(size_t)sy * cpitch + sx] = val;
+            }
         }
     }
     __syncthreads();
@@ -83,18 +97,18 @@ __global__ void __launch_bounds__(256) k1_pyramid_down(const float *__restrict__
         s = fmaf(0.375f, p[2], s);
         s = fmaf(0.25f, p[3], s);
         s = fmaf(0.0625f, p[4], s);
-        T[r][X] = s;
+        T_[r][X] = s;
     }
     __syncthreads();
     {
         int X = threadIdx.x & (K1_TW - 1), Y = threadIdx.x / K1_TW;
         int gx = X0 + X, gy = Y0 + Y;
         if (gx < Wd && gy < Hd) {
-            float s = 0.0625f * T[2 * Y][X];
-            s = fmaf(0.25f, T[2 * Y + 1][X], s);
-            s = fmaf(0.375f, T[2 * Y + 2][X], s);
-            s = fmaf(0.25f, T[2 * Y + 3][X], s);
-            s = fmaf(0.0625f, T[2 * Y + 4][X], s);
+            float s = 0.0625f * T_[2 * Y][X];
+            s = fmaf(0.25f, T_[2 * Y + 1][X], s);
+            s = fmaf(0.375f, T_[2 * Y + 2][X], s);
+            s = fmaf(0.25f, T_[2 * Y + 3][X], s);
+            s = fmaf(0.0625f, T_[2 * Y + 4][X], s);
             dst[(size_t)gy * dpitch + gx] = s;
         }
     }

@@ -299,7 +299,20 @@ void run_pyramid(const of_context *c, int l, const float *sa, const float *sb, f
 {
     const Level &S = c->lv[l], &D = c->lv[l + 1];
     dim3 grid((D.W + K1_TW - 1) / K1_TW, (D.H + K1_TH - 1) / K1_TH, sb ? 2 : 1);
-    k1_pyramid_down<<<grid, 256, 0, st>>>(sa, sb, da, db, S.W, S.H, S.pitch, D.W, D.H, D.pitch);
+    k1_pyramid_down<float><<<grid, 256, 0, st>>>(sa, sb, da, db, S.W, S.H, S.pitch, D.W, D.H, D.pitch, nullptr, nullptr, 0);
+}
+
+// First pyramid step fused with the frame conversion: raw frame -> fp32 level 0 AND level 1 in one kernel.
+void run_convert_pyramid(const of_context *c, int dtype, const void *a, const void *b, float *a0, float *b0, float *a1, float *b1, cudaStream_t st)
+{
+    const Level &S = c->lv[0], &D = c->lv[1];
+    dim3 grid((D.W + K1_TW - 1) / K1_TW, (D.H + K1_TH - 1) / K1_TH, b ? 2 : 1);
+    if (dtype == OF_DTYPE_U8)
+        k1_pyramid_down<uint8_t><<<grid, 256, 0, st>>>((const uint8_t *)a, (const uint8_t *)b, a1, b1, S.W, S.H, S.W, D.W, D.H, D.pitch, a0, b0, S.pitch);
+    else if (dtype == OF_DTYPE_U16)
+        k1_pyramid_down<uint16_t><<<grid, 256, 0, st>>>((const uint16_t *)a, (const uint16_t *)b, a1, b1, S.W, S.H, S.W, D.W, D.H, D.pitch, a0, b0, S.pitch);
+    else
+        k1_pyramid_down<float><<<grid, 256, 0, st>>>((const float *)a, (const float *)b, a1, b1, S.W, S.H, S.W, D.W, D.H, D.pitch, a0, b0, S.pitch);
 }
 
 void run_upsample(const of_context *c, int l, cudaStream_t st)   // level l+1 -> l
@@ -326,10 +339,19 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
     c->launch_err.clear();
     if (j.cvtA >= 0) {
         const bool both = j.cvtB >= 0;
-        run_convert(c, j.dtype, j.rawA, both ? j.rawB : nullptr, c->pyr[j.cvtA][0], both ? c->pyr[j.cvtB][0] : nullptr, st);
-        note_launch(c, "convert", 0);
-        ++n;
-        for (int l = 0; l + 1 < c->levels; ++l) {
+        int l0 = 0;
+        if (c->levels > 1 && c->eq_radius == 0) {               // conversion fused into the first pyramid step
+            run_convert_pyramid(c, j.dtype, j.rawA, both ? j.rawB : nullptr, c->pyr[j.cvtA][0], both ? c->pyr[j.cvtB][0] : nullptr,
+                                c->pyr[j.cvtA][1], both ? c->pyr[j.cvtB][1] : nullptr, st);
+            note_launch(c, "convert+pyramid", 0);
+            ++n;
+            l0 = 1;
+        } else {
+            run_convert(c, j.dtype, j.rawA, both ? j.rawB : nullptr, c->pyr[j.cvtA][0], both ? c->pyr[j.cvtB][0] : nullptr, st);
+            note_launch(c, "convert", 0);
+            ++n;
+        }
+        for (int l = l0; l + 1 < c->levels; ++l) {
             run_pyramid(c, l, c->pyr[j.cvtA][l], both ? c->pyr[j.cvtB][l] : nullptr, c->pyr[j.cvtA][l + 1],
                         both ? c->pyr[j.cvtB][l + 1] : nullptr, st);
             note_launch(c, "pyramid", l);
@@ -757,7 +779,7 @@ int of_pyramid_down(const float *src, int width, int height, float *dst, void *s
     if (!src || !dst || width < 1 || height < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
     int Wd = (width + 1) / 2, Hd = (height + 1) / 2;
     dim3 grid((Wd + K1_TW - 1) / K1_TW, (Hd + K1_TH - 1) / K1_TH, 1);
-    k1_pyramid_down<<<grid, 256, 0, (cudaStream_t)stream>>>(src, nullptr, dst, nullptr, width, height, width, Wd, Hd, Wd);
+    k1_pyramid_down<float><<<grid, 256, 0, (cudaStream_t)stream>>>(src, nullptr, dst, nullptr, width, height, width, Wd, Hd, Wd, nullptr, nullptr, 0);
     CU_TRY(cudaGetLastError());
     return OF_OK;
 }

@@ -288,7 +288,7 @@ def test_graph_and_plain_launches_agree_bitwise_and_repeat(torch, B):
     a = gpu_solve(torch, B, c.I1, c.I2, 3, 12, 4, GAUSS, graph=True)
     b = gpu_solve(torch, B, c.I1, c.I2, 3, 12, 4, GAUSS, graph=False)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
-    assert a[3] == b[3] == 1 + 2 + 1                      # convert, 2 pyramid steps, 1 persistent solve
+    assert a[3] == b[3] == 2 + 1                          # convert+pyramid, pyramid, 1 persistent solve
     H, W = c.I1.shape
     with B.OpticalFlow(W, H, 3, 12, 4, GAUSS) as of:
         d1, d2 = torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()
@@ -320,7 +320,8 @@ def test_persistent_and_per_kernel_launches_agree_bitwise(torch, B, W, H, L, R, 
             s.synchronize()
             out.append((u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy(), of.last_launch_count()))
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2])
-    assert out[0][3] == 1 + (L - 1) + 1 and out[1][3] == 1 + 2 * (L - 1) + 2 * L * it
+    prep = 1 if L == 1 else L - 1                          # conversion is fused into the first pyramid step
+    assert out[0][3] == prep + 1 and out[1][3] == prep + (L - 1) + 2 * L * it
 
 
 def test_large_image_crop_parity(torch, B, oracle):

@@ -50,11 +50,13 @@ __global__ void __launch_bounds__(256) k0_convert(const T *__restrict__ srcA, co
 
 // ------------------------------------------------------------------------------------------------
 // K1: pyramid step (row a2; "reduced in size by a factor of 4"; D4, D5).
-// CTA = 32x8 outputs; source patch (2*32+3) x (2*8+3) staged in shared memory with clamped indices,
+// CTA = 32 x K1_TH outputs; source patch (2*32+3) x (2*K1_TH+3) staged in shared memory with clamped indices,
 // rows filtered first, then columns (same order as the definition).
 // ------------------------------------------------------------------------------------------------
 #define K1_TW 32                                   // (the index arithmetic below relies on K1_TW == 32)
+#ifndef K1_TH
 #define K1_TH 8
+#endif
 // T = float: level l -> l+1 of an fp32 pyramid.  T = uint8_t / uint16_t / float with cvtA/cvtB != NULL: the first
 // step of a pair, fused with the frame conversion (row a1): the source is the raw dense frame (pitch == W) and
 // every CTA also writes the fp32 level-0 plane for the core of its patch (each source pixel belongs to exactly
@@ -100,9 +102,9 @@ __global__ void __launch_bounds__(256) k1_pyramid_down(const T *__restrict__ src
         T_[r][X] = s;
     }
     __syncthreads();
-    {
-        int X = threadIdx.x & (K1_TW - 1), Y = threadIdx.x / K1_TW;
-        int gx = X0 + X, gy = Y0 + Y;
+    for (int i = threadIdx.x; i < K1_TW * K1_TH; i += 256) {
+        const int X = i & (K1_TW - 1), Y = i / K1_TW;
+        const int gx = X0 + X, gy = Y0 + Y;
         if (gx < Wd && gy < Hd) {
             float s = 0.0625f * T_[2 * Y][X];
             s = fmaf(0.25f, T_[2 * Y + 1][X], s);

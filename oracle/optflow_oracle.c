@@ -25,6 +25,9 @@
  * exactness on constants and ramps; eq. 1 behaviour; monotone error vs iterations
  * (Table 1 trend); oracle_equalise (eq. 2): zero local mean / unit local variance,
  * gain-offset invariance, flat image -> 0, agreement with scipy uniform_filter in the interior.
+ * Masks (f4, readings M1-M5 above oracle_mask_downsample): all-ones mask == no mask bit for bit; ramp
+ * still exact in one iteration at every fluid pixel; the sums equal brute-force sums of mask*product;
+ * image content deep under the mask does not reach any fluid vector; mask pyramid vs a Python loop.
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -195,9 +198,9 @@ void oracle_window_sum(const double *f, int W, int H, int R, int window_type, do
  * u, v are updated in place at the end.  sums5 (optional) receives a,b,c,p,q as 5 planes; valid
  * (optional) the validity bytes; det (optional) the undamped a*c - b^2.
  * direct_sums != 0 uses oracle_window_sum_direct instead of the two-pass form. */
-void oracle_iteration(const double *I1, const double *I2, int W, int H, int R, int window_type,
-                      double eps, double max_step, double *u, double *v, double *sums5,
-                      unsigned char *valid, double *det, int direct_sums)
+void oracle_iteration_masked(const double *I1, const double *I2, const unsigned char *mask, int W, int H, int R,
+                             int window_type, double eps, double max_step, double *u, double *v, double *sums5,
+                             unsigned char *valid, double *det, int direct_sums)
 {
     size_t N = (size_t)W * H;
     double *I2w = (double *)malloc(sizeof(double) * N);
@@ -216,6 +219,8 @@ void oracle_iteration(const double *I1, const double *I2, int W, int H, int R, i
         prod[2 * N + k] = Iy[k] * Iy[k];
         prod[3 * N + k] = Ix[k] * It;
         prod[4 * N + k] = Iy[k] * It;
+        if (mask && !mask[k])                       /* M2: an obstacle pixel has zero weight in every window sum */
+            for (int f = 0; f < 5; ++f) prod[f * N + k] = 0.0;
     }
     for (int f = 0; f < 5; ++f) {
         if (direct_sums) oracle_window_sum_direct(prod + f * N, W, H, R, window_type, S + f * N);
@@ -241,9 +246,46 @@ void oracle_iteration(const double *I1, const double *I2, int W, int H, int R, i
         v[k] += dv;
         if (valid) valid[k] = ok;
         if (det) det[k] = a * c - b * b;
+        if (mask && !mask[k]) {                     /* M3: no vector over an obstacle */
+            u[k] = 0.0; v[k] = 0.0;
+            if (valid) valid[k] = 0;
+            if (det) det[k] = 0.0;
+        }
     }
     if (sums5) memcpy(sums5, S, sizeof(double) * N * 5);
     free(S); free(prod); free(Iy); free(Ix); free(I2w);
+}
+
+void oracle_iteration(const double *I1, const double *I2, int W, int H, int R, int window_type,
+                      double eps, double max_step, double *u, double *v, double *sums5,
+                      unsigned char *valid, double *det, int direct_sums)
+{
+    oracle_iteration_masked(I1, I2, NULL, W, H, R, window_type, eps, max_step, u, v, sums5, valid, det, direct_sums);
+}
+
+/* NEXT item f4: masks over obstacles and side walls ("using masks to avoid
+ * computations over obstacles or side walls").  The paper gives no more than that sentence; readings:
+ *   M1 the mask is one byte per level-0 pixel, non-zero = fluid (computed), 0 = obstacle;
+ *   M2 an obstacle pixel has zero weight in every window sum (its five products are dropped);
+ *   M3 an obstacle pixel carries no vector: u = v = 0, valid = 0, det = 0, at every level and at every
+ *      moment of the solve (after each update and after the hand-down);
+ *   M4 level l+1 pixel (X,Y) is fluid iff at least one of its in-image children (2X..2X+1, 2Y..2Y+1) is;
+ *   M5 the images themselves are not altered (the pyramid filter, the gradients and the warp read
+ *      obstacle pixels as they are).
+ * This function is M4. */
+void oracle_mask_downsample(const unsigned char *src, int W, int H, unsigned char *dst)
+{
+    int Wd = (W + 1) / 2, Hd = (H + 1) / 2;
+    for (int Y = 0; Y < Hd; ++Y)
+        for (int X = 0; X < Wd; ++X) {
+            int any = 0;
+            for (int dy = 0; dy < 2; ++dy)
+                for (int dx = 0; dx < 2; ++dx) {
+                    int x = 2 * X + dx, y = 2 * Y + dy;
+                    if (x < W && y < H && src[(size_t)y * W + x]) any = 1;
+                }
+            dst[(size_t)Y * Wd + X] = (unsigned char)any;
+        }
 }
 
 /* The whole solve O1..O5.  I1, I2: level-0 images as doubles (exact conversion of the integer
@@ -251,10 +293,10 @@ void oracle_iteration(const double *I1, const double *I2, int W, int H, int R, i
  * valid and det (optional) from the last iteration of level 0.
  * level_u / level_v (optional): arrays of `levels` pointers, each receiving that level's final field.
  * Returns 0, or -1 on bad arguments (coarsest level smaller than the window). */
-int oracle_solve(const double *I1, const double *I2, int W, int H, int levels, int R, int iterations,
-                 int window_type, double eps, double max_step, double *u, double *v,
-                 unsigned char *valid, double *det, double **level_u, double **level_v,
-                 int direct_sums)
+int oracle_solve_masked(const double *I1, const double *I2, const unsigned char *mask, int W, int H, int levels,
+                        int R, int iterations, int window_type, double eps, double max_step, double *u, double *v,
+                        unsigned char *valid, double *det, double **level_u, double **level_v,
+                        int direct_sums)
 {
     if (W < 1 || H < 1 || levels < 1 || levels > 16 || R < 1 || iterations < 1) return -1;
     int Ws[16], Hs[16];
@@ -270,6 +312,15 @@ int oracle_solve(const double *I1, const double *I2, int W, int H, int levels, i
         oracle_downsample(P1[l - 1], Ws[l - 1], Hs[l - 1], P1[l]);
         oracle_downsample(P2[l - 1], Ws[l - 1], Hs[l - 1], P2[l]);
     }
+    unsigned char *M[16];                 /* mask == NULL: no mask at any level */
+    M[0] = (unsigned char *)mask;
+    for (int l = 1; l < levels; ++l) {
+        M[l] = NULL;
+        if (mask) {
+            M[l] = (unsigned char *)malloc((size_t)Ws[l] * Hs[l]);
+            oracle_mask_downsample(M[l - 1], Ws[l - 1], Hs[l - 1], M[l]);
+        }
+    }
     double *uc = NULL, *vc = NULL;        /* field of the level just finished */
     for (int l = levels - 1; l >= 0; --l) {
         size_t N = (size_t)Ws[l] * Hs[l];
@@ -279,10 +330,13 @@ int oracle_solve(const double *I1, const double *I2, int W, int H, int levels, i
             oracle_upsample_flow(uc, Ws[l + 1], Hs[l + 1], ul, Ws[l], Hs[l]);
             oracle_upsample_flow(vc, Ws[l + 1], Hs[l + 1], vl, Ws[l], Hs[l]);
             free(uc); free(vc);
+            if (M[l])                                       /* M3 */
+                for (size_t k = 0; k < N; ++k)
+                    if (!M[l][k]) { ul[k] = 0.0; vl[k] = 0.0; }
         }
         for (int n = 0; n < iterations; ++n)
-            oracle_iteration(P1[l], P2[l], Ws[l], Hs[l], R, window_type, eps, max_step, ul, vl, NULL,
-                             (l == 0) ? valid : NULL, (l == 0) ? det : NULL, direct_sums);
+            oracle_iteration_masked(P1[l], P2[l], M[l], Ws[l], Hs[l], R, window_type, eps, max_step, ul, vl, NULL,
+                                    (l == 0) ? valid : NULL, (l == 0) ? det : NULL, direct_sums);
         if (level_u && level_u[l]) memcpy(level_u[l], ul, sizeof(double) * N);
         if (level_v && level_v[l]) memcpy(level_v[l], vl, sizeof(double) * N);
         uc = ul; vc = vl;
@@ -290,8 +344,17 @@ int oracle_solve(const double *I1, const double *I2, int W, int H, int levels, i
     memcpy(u, uc, sizeof(double) * (size_t)W * H);
     memcpy(v, vc, sizeof(double) * (size_t)W * H);
     free(uc); free(vc);
-    for (int l = 1; l < levels; ++l) { free(P1[l]); free(P2[l]); }
+    for (int l = 1; l < levels; ++l) { free(P1[l]); free(P2[l]); free(M[l]); }
     return 0;
+}
+
+int oracle_solve(const double *I1, const double *I2, int W, int H, int levels, int R, int iterations,
+                 int window_type, double eps, double max_step, double *u, double *v,
+                 unsigned char *valid, double *det, double **level_u, double **level_v,
+                 int direct_sums)
+{
+    return oracle_solve_masked(I1, I2, NULL, W, H, levels, R, iterations, window_type, eps, max_step, u, v,
+                               valid, det, level_u, level_v, direct_sums);
 }
 
 /* NEXT item f1: local equalisation pre-filter, eq. 2 of the paper:

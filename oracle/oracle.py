@@ -41,6 +41,7 @@ def lib():
         _lib.oracle_window_weight.restype = ctypes.c_double
         _lib.oracle_window_weight.argtypes = [ctypes.c_int] * 3
         _lib.oracle_solve.restype = ctypes.c_int
+        _lib.oracle_solve_masked.restype = ctypes.c_int
         _lib.oracle_num_threads.restype = ctypes.c_int
     return _lib
 
@@ -113,17 +114,37 @@ def window_sum(f, R, window_type, direct=False):
     return out
 
 
-def iteration(I1, I2, u, v, R, window_type, eps=EPS_REL, max_step=MAX_STEP, direct=False):
-    """One iteration; returns (u_new, v_new, sums5[5,H,W], valid[H,W] uint8, det[H,W])."""
+def _mask(mask, shape):
+    if mask is None:
+        return None, None
+    m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.uint8)
+    assert m.shape == shape
+    return m, m.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte))
+
+
+def mask_downsample(mask):
+    """One step of the mask pyramid (reading M4): fluid iff any in-image child is fluid."""
+    m, pm = _mask(mask, np.asarray(mask).shape)
+    H, W = m.shape
+    out = np.empty(((H + 1) // 2, (W + 1) // 2), dtype=np.uint8)
+    lib().oracle_mask_downsample(pm, ctypes.c_int(W), ctypes.c_int(H),
+                                 out.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)))
+    return out
+
+
+def iteration(I1, I2, u, v, R, window_type, eps=EPS_REL, max_step=MAX_STEP, direct=False, mask=None):
+    """One iteration; returns (u_new, v_new, sums5[5,H,W], valid[H,W] uint8, det[H,W]).
+    mask (optional, f4): non-zero = fluid, readings M1-M3."""
     a, pa = _d(I1)
     b, pb = _d(I2)
     H, W = a.shape
+    m, pm = _mask(mask, a.shape)
     un = np.array(u, dtype=np.float64, order="C", copy=True)
     vn = np.array(v, dtype=np.float64, order="C", copy=True)
     sums = np.empty((5, H, W))
     valid = np.empty((H, W), dtype=np.uint8)
     det = np.empty((H, W))
-    lib().oracle_iteration(pa, pb, ctypes.c_int(W), ctypes.c_int(H), ctypes.c_int(R),
+    lib().oracle_iteration_masked(pa, pb, pm, ctypes.c_int(W), ctypes.c_int(H), ctypes.c_int(R),
                            ctypes.c_int(window_type), ctypes.c_double(eps), ctypes.c_double(max_step),
                            un.ctypes.data_as(_dp), vn.ctypes.data_as(_dp), sums.ctypes.data_as(_dp),
                            valid.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)),
@@ -132,12 +153,14 @@ def iteration(I1, I2, u, v, R, window_type, eps=EPS_REL, max_step=MAX_STEP, dire
 
 
 def solve(I1, I2, levels, R, iterations, window_type, eps=EPS_REL, max_step=MAX_STEP,
-          direct=False, return_levels=False):
-    """Whole solve.  Returns dict(u, v, valid, det[, level_u, level_v])."""
+          direct=False, return_levels=False, mask=None):
+    """Whole solve.  Returns dict(u, v, valid, det[, level_u, level_v]).
+    mask (optional, f4): level-0 bytes, non-zero = fluid, readings M1-M5."""
     a, pa = _d(I1)
     b, pb = _d(I2)
     assert a.shape == b.shape and a.ndim == 2
     H, W = a.shape
+    m, pm = _mask(mask, a.shape)
     u, v = np.empty((H, W)), np.empty((H, W))
     valid = np.empty((H, W), dtype=np.uint8)
     det = np.empty((H, W))
@@ -152,7 +175,7 @@ def solve(I1, I2, levels, R, iterations, window_type, eps=EPS_REL, max_step=MAX_
             w, h = (w + 1) // 2, (h + 1) // 2
         plu = (_dp * levels)(*[x.ctypes.data_as(_dp) for x in lu])
         plv = (_dp * levels)(*[x.ctypes.data_as(_dp) for x in lv])
-    rc = lib().oracle_solve(pa, pb, ctypes.c_int(W), ctypes.c_int(H), ctypes.c_int(levels),
+    rc = lib().oracle_solve_masked(pa, pb, pm, ctypes.c_int(W), ctypes.c_int(H), ctypes.c_int(levels),
                             ctypes.c_int(R), ctypes.c_int(iterations), ctypes.c_int(window_type),
                             ctypes.c_double(eps), ctypes.c_double(max_step),
                             u.ctypes.data_as(_dp), v.ctypes.data_as(_dp),

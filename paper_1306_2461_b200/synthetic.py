@@ -134,6 +134,18 @@ def field_backward_step(width, height):
     return d
 
 
+def mask_backward_step(width, height):
+    """Obstacle mask (uint8, 1 = fluid, 0 = obstacle) for the NEXT item f4 (PAPER.md:175 'masks to avoid
+    computations over obstacles or side walls'): the step body (x < 0.25 W below the shear layer at
+    y = 0.6 H) and two side-wall bands of 3 percent of the height.  About 14 percent of the frame."""
+    m = np.ones((height, width), dtype=np.uint8)
+    wall = max(1, int(round(0.03 * height)))
+    m[:wall, :] = 0
+    m[height - wall:, :] = 0
+    m[int(round(0.6 * height)):, :int(round(0.25 * width))] = 0
+    return m
+
+
 def field_random_smooth(rng, width, height, filt_sigma, rms, pad=64):
     """Two independent white-noise fields, Gaussian-filtered (FFT) on a padded grid, jointly scaled
     to sqrt(mean(u^2+v^2)) = rms over the image; evaluated off-grid by cubic splines."""

@@ -457,3 +457,145 @@ def test_bubble_surface_of_the_backward_step_like_truth_field(oracle):
     below, total = oracle.bubble_counts(c.truth_u, T)
     assert total == 320 * 256 and below == int(np.count_nonzero(c.truth_u <= T))
     assert 0.15 < below / total < 0.45
+
+
+# ---------------------------------------------------------------------------- masks (NEXT item f4)
+# PAPER.md:175 "using masks to avoid computations over obstacles or side walls"; readings M1-M5
+# (oracle/optflow_oracle.c above oracle_mask_downsample).
+def _blob_mask(H, W):
+    m = np.ones((H, W), dtype=np.uint8)
+    m[20:44, 10:40] = 0          # an obstacle
+    m[:, :3] = 0                 # a side wall
+    m[50, 60] = 0                # a single dead pixel
+    return m
+
+
+def test_mask_of_ones_is_no_mask_bit_for_bit(oracle):
+    c = syn.config2(96, 80)
+    a = oracle.solve(c.I1, c.I2, 2, 5, 2, GAUSS)
+    b = oracle.solve(c.I1, c.I2, 2, 5, 2, GAUSS, mask=np.ones((80, 96), dtype=np.uint8))
+    for k in ("u", "v", "valid", "det"):
+        assert np.array_equal(a[k], b[k])
+
+
+def test_masked_pixels_carry_no_vector_at_any_level(oracle):
+    """M3: u = v = 0, valid = 0, det = 0 over the obstacle, at every level (mask pyramid M4)."""
+    c = syn.config2(96, 80)
+    m0 = _blob_mask(80, 96)
+    r = oracle.solve(c.I1, c.I2, 3, 4, 2, BOX, mask=m0, return_levels=True)
+    m = m0
+    for l in range(3):
+        assert np.all(r["level_u"][l][m == 0] == 0.0) and np.all(r["level_v"][l][m == 0] == 0.0)
+        assert np.any(r["level_u"][l][m == 1] != 0.0)
+        m = oracle.mask_downsample(m)
+    assert np.all(r["valid"][m0 == 0] == 0) and np.all(r["det"][m0 == 0] == 0.0)
+    assert r["valid"][m0 == 1].min() == 1          # textured fluid pixels stay valid next to the obstacle
+
+
+def test_mask_pyramid_is_the_or_of_the_children(oracle):
+    """M4 against a plain Python loop, odd sizes (last column / row has fewer children)."""
+    rng = np.random.default_rng(5)
+    m = (rng.random((13, 17)) < 0.3).astype(np.uint8)
+    got = oracle.mask_downsample(m)
+    assert got.shape == (7, 9)
+    for Y in range(7):
+        for X in range(9):
+            kids = [m[y, x] for y in (2 * Y, 2 * Y + 1) for x in (2 * X, 2 * X + 1) if y < 13 and x < 17]
+            assert got[Y, X] == (1 if any(kids) else 0)
+    assert oracle.mask_downsample(np.zeros((4, 6), np.uint8)).max() == 0
+    assert oracle.mask_downsample(np.ones((5, 5), np.uint8)).min() == 1
+
+
+@pytest.mark.parametrize("wt,R", [(BOX, 3), (GAUSS, 6)])
+def test_masked_sums_are_brute_force_sums_of_mask_times_product(oracle, wt, R):
+    """M2: a, b, c, p, q = sum over the window of w * mask * product, summed pixel by pixel here from
+    the oracle's own warp / gradient primitives (32x32, zero extension outside the image)."""
+    rng = np.random.default_rng(9)
+    I1 = rng.random((32, 32)) * 100.0
+    I2 = rng.random((32, 32)) * 100.0
+    u = rng.normal(0.0, 0.7, (32, 32))
+    v = rng.normal(0.0, 0.7, (32, 32))
+    m = (rng.random((32, 32)) < 0.6).astype(np.uint8)
+    _, _, sums, valid, _ = oracle.iteration(I1, I2, u, v, R, wt, mask=m)
+    Ix, Iy = oracle.gradients(I1)
+    It = oracle.warp(I2, u, v) - I1 - Ix * u - Iy * v
+    prods = [Ix * Ix, Ix * Iy, Iy * Iy, Ix * It, Iy * It]
+    w = [oracle.window_weight(t, R, wt) for t in range(-R, R + 1)]
+    for (y, x) in [(0, 0), (5, 17), (31, 31), (16, 2), (30, 9)]:
+        for f in range(5):
+            acc = 0.0
+            for dy in range(-R, R + 1):
+                for dx in range(-R, R + 1):
+                    yy, xx = y + dy, x + dx
+                    if 0 <= yy < 32 and 0 <= xx < 32 and m[yy, xx]:
+                        acc += w[dy + R] * w[dx + R] * prods[f][yy, xx]
+            assert abs(sums[f, y, x] - acc) <= 1e-9 * max(1.0, abs(acc))
+    assert np.all(valid[m == 0] == 0)
+
+
+def test_ramp_is_still_solved_in_one_iteration_beside_an_obstacle(oracle):
+    """Every pixel of a linear ramp satisfies the same linear equation, so dropping any subset of them
+    from the window (M2) leaves the closed form u = d/(1+eps/2) at every fluid pixel whose window
+    still holds a fluid pixel.  A mask applied to G but not to the right-hand side (or the reverse)
+    fails this."""
+    I1, I2, d = syn.ramp_pair(64, 64, (0.8, 0.6), 0.25)
+    m = np.ones((64, 64), dtype=np.uint8)
+    m[24:40, 20:50] = 0
+    m[10, 10] = 0
+    z = np.zeros_like(I1)
+    eps = 1e-3
+    u, v, _, valid, _ = oracle.iteration(I1, I2, z, z, 6, BOX, eps=eps, mask=m)
+    k = 1.0 / (1.0 + eps / 2.0)
+    fluid = interior(m, 8) == 1
+    assert np.max(np.abs(interior(u, 8)[fluid] - d[0] * k)) < 2e-12
+    assert np.max(np.abs(interior(v, 8)[fluid] - d[1] * k)) < 2e-12
+    assert np.all(u[m == 0] == 0.0) and np.all(valid[m == 0] == 0) and np.all(valid[m == 1] == 1)
+
+
+def test_image_content_deep_under_the_mask_reaches_no_fluid_vector(oracle):
+    """M2 + M5 at one level: a fluid vector depends on the images only through fluid pixels of its
+    window, their gradient stencils (1 px) and their warped samples (|u| <= iterations * 3 px, D15).
+    Scribbling over the obstacle's deep interior leaves every fluid vector bit-identical with the mask
+    and changes vectors near the obstacle without it."""
+    c = syn.config1(96, 96)
+    I1, I2 = c.I1.astype(np.float64), c.I2.astype(np.float64)
+    m = np.ones((96, 96), dtype=np.uint8)
+    m[20:76, 30:70] = 0
+    J1, J2 = I1.copy(), I2.copy()
+    rng = np.random.default_rng(3)
+    J1[30:66, 40:60] = rng.random((36, 20)) * 255.0      # >= 10 px from any fluid pixel
+    J2[30:66, 40:60] = rng.random((36, 20)) * 255.0
+    a = oracle.solve(I1, I2, 1, 8, 2, BOX, mask=m)
+    b = oracle.solve(J1, J2, 1, 8, 2, BOX, mask=m)
+    assert np.array_equal(a["u"], b["u"]) and np.array_equal(a["v"], b["v"]) and np.array_equal(a["valid"], b["valid"])
+    a0 = oracle.solve(I1, I2, 1, 8, 2, BOX)
+    b0 = oracle.solve(J1, J2, 1, 8, 2, BOX)
+    assert np.max(np.abs(a0["u"] - b0["u"])[m == 1]) > 1e-3
+
+
+def test_masked_solve_equals_stepwise_composition(oracle):
+    """Two levels with a mask: pyramid of images and of masks, masked iterations, hand-down, zero over
+    the obstacle (M3), masked iterations -- composed from the primitives."""
+    c = syn.config2(96, 80)
+    I1, I2 = c.I1.astype(np.float64), c.I2.astype(np.float64)
+    m0 = _blob_mask(80, 96)
+    m1 = oracle.mask_downsample(m0)
+    r = oracle.solve(I1, I2, 2, 5, 2, GAUSS, mask=m0)
+    P1, P2 = oracle.downsample(I1), oracle.downsample(I2)
+    u = np.zeros_like(P1)
+    v = np.zeros_like(P1)
+    for _ in range(2):
+        u, v, *_ = oracle.iteration(P1, P2, u, v, 5, GAUSS, mask=m1)
+    u, v = oracle.upsample_flow(u, 96, 80), oracle.upsample_flow(v, 96, 80)
+    u[m0 == 0] = 0.0
+    v[m0 == 0] = 0.0
+    for _ in range(2):
+        u, v, s, valid, det = oracle.iteration(I1, I2, u, v, 5, GAUSS, mask=m0)
+    assert np.array_equal(u, r["u"]) and np.array_equal(v, r["v"]) and np.array_equal(valid, r["valid"])
+
+
+def test_backward_step_mask_recipe():
+    m = syn.mask_backward_step(1280, 1024)
+    assert m.dtype == np.uint8 and m.shape == (1024, 1280)
+    assert 0.13 < 1.0 - m.mean() < 0.17
+    assert m[512, 640] == 1 and m[0, 0] == 0 and m[1000, 100] == 0

@@ -87,6 +87,16 @@ int of_set_conditioning(of_handle h, float eps_rel, float max_step_px);
  * conversion (it replaces that kernel).  radius 0 (default) switches it off; the paper uses 5. */
 int of_set_equalisation(of_handle h, int radius);
 
+/* Obstacle mask ("using masks to avoid computations over obstacles or side walls").
+ * mask_host: HOST pointer to height rows of row_stride (>= width) bytes, non-zero = fluid, 0 = obstacle;
+ * copied and preprocessed by this call (the caller keeps ownership); NULL removes the mask.  A set-up
+ * call: it synchronises the device and must not overlap a solve on this handle.  Readings (DESIGN.md
+ * M1-M5): an obstacle pixel has zero weight in every window sum and carries no vector (u = v = 0,
+ * valid = 0, at every level); a coarse pixel is an obstacle iff all its in-image children are; the
+ * images themselves are not altered.  Tiles and tasks that neither hold nor feed a fluid pixel are
+ * skipped and the remaining work is re-balanced over the SMs.  Returns OF_OK or an error code. */
+int of_set_mask(of_handle h, const uint8_t *mask_host, int row_stride);
+
 /* Replay the per-pair launch sequence as a CUDA graph (default on).  The graph is re-captured when
  * the caller's pointers change. */
 int of_set_graph(of_handle h, int enable);

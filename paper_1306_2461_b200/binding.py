@@ -30,6 +30,7 @@ SIGNATURES = {
     "of_last_error": (_c.c_char_p, []),
     "of_set_conditioning": (_i, [_vp, _c.c_float, _c.c_float]),
     "of_set_equalisation": (_i, [_vp, _i]),
+    "of_set_mask": (_i, [_vp, _vp, _i]),
     "of_set_graph": (_i, [_vp, _i]),
     "of_set_persistent": (_i, [_vp, _i]),
     "of_solve_timeline": (_i, [_vp, _i, _i, _vp, _i]),
@@ -150,6 +151,17 @@ class OpticalFlow:
 
     def set_equalisation(self, radius: int):
         _check(lib().of_set_equalisation(self._h, int(radius)))
+
+    def set_mask(self, mask):
+        """Obstacle mask: HxW array, non-zero = fluid; None removes it.  Set-up call (synchronises)."""
+        if mask is None:
+            _check(lib().of_set_mask(self._h, None, 0))
+            return
+        import numpy as np
+        m = np.ascontiguousarray(np.asarray(mask.cpu() if hasattr(mask, "cpu") else mask) != 0, dtype=np.uint8)
+        if m.shape != (self.height, self.width):
+            raise ValueError("mask must be %dx%d" % (self.height, self.width))
+        _check(lib().of_set_mask(self._h, m.ctypes.data, self.width))
 
     def set_graph(self, enable: bool):
         _check(lib().of_set_graph(self._h, 1 if enable else 0))

@@ -43,6 +43,8 @@ struct K2Params {
     int zero_uv;                                   // 1 = the field is identically zero (first iteration at the coarsest level,
                                                    // PAPER.md:61 "initial guess of zero displacement"): u, v are not read
     int dbg;                                       // profiling switches (0 in production): 1 = no product phase, 2 = no sum phase, 32 = no plane stores
+    const uint8_t *mask;                           // obstacle mask of the level (pitch = `pitch`) or NULL (M2: zero weight)
+    const int *list;                               // compacted tile list (then ntiles = its length) or NULL
 };
 
 // Inputs of one phase-1 task (2 columns x 2 rows): I1 rows y-1..y+2 at columns x, x+1, the left and
@@ -52,6 +54,7 @@ struct K2Params {
 struct K2In {
     float2 cm, c0, c1, c2, u0, u1, v0, v1;
     float l0, q0, l1, q1;
+    unsigned m0, m1;                               // mask bytes of (x, x+1) in rows y, y+1 (only read when a mask is set)
 };
 
 // base + 4*idx as ONE IMAD.WIDE (FMA pipe).  The integer/compare pipe (16 lanes per clock per SM sub-partition)
@@ -63,7 +66,7 @@ __device__ __forceinline__ const float *ptr_at(const float *base, int idx)
     return r;
 }
 
-__device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
+template <bool MK> __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
 {
     K2In in;
     const int W = p.W, H = p.H, pitch = p.pitch;
@@ -82,6 +85,12 @@ __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
         in.u1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pu, d1)));
         in.v0 = __ldcg(reinterpret_cast<const float2 *>(pv));
         in.v1 = __ldcg(reinterpret_cast<const float2 *>(ptr_at(pv, d1)));
+    }
+    in.m0 = in.m1 = 0x0101u;
+    if (MK) {
+        const uint8_t *pm = p.mask + i0;           // x is even and the pitch a multiple of 32: 2-byte aligned
+        in.m0 = __ldg(reinterpret_cast<const unsigned short *>(pm));
+        in.m1 = __ldg(reinterpret_cast<const unsigned short *>(pm + d1));
     }
     // left / right neighbours with clamp-to-edge: x-1 -> x at the left border, x+2 -> W-1 at the right
     const int ol = x > 0 ? -1 : 0, orr = x + 2 < W ? 2 : (x + 1 < W ? 1 : 0);
@@ -145,11 +154,15 @@ __device__ __forceinline__ void k2_products(float I2w, float uu, float vv, float
     xx = gx * gx; xy = gx * gy; yy = gy * gy; xt = gx * It; yt = gy * It;
 }
 
-__device__ __forceinline__ void k2_task_products(const K2Params &p, const K2In &cur, int x, int y, const K2Tap (&t)[4], float4 (&o)[5])
+template <bool MK> __device__ __forceinline__ void k2_task_products(const K2Params &p, const K2In &cur, int x, int y, const K2Tap (&t)[4], float4 (&o)[5])
 {
     const bool in1 = x + 1 < p.W, row1 = y + 1 < p.H;
-    const float m01 = in1 ? 0.5f : 0.f, m10 = row1 ? 0.5f : 0.f, m11 = (in1 && row1) ? 0.5f : 0.f;
-    k2_products(k2_lerp(t[0]), cur.u0.x, cur.v0.x, cur.c0.x, 0.5f * ((in1 ? cur.c0.y : cur.c0.x) - cur.l0), 0.5f * (cur.c1.x - cur.cm.x),
+    float m00 = 0.5f, m01 = in1 ? 0.5f : 0.f, m10 = row1 ? 0.5f : 0.f, m11 = (in1 && row1) ? 0.5f : 0.f;
+    if (MK) {                                      // M2: an obstacle pixel gets zero gradients, hence five zero products
+        m00 = (cur.m0 & 0xffu) ? m00 : 0.f; m01 = (cur.m0 >> 8) ? m01 : 0.f;
+        m10 = (cur.m1 & 0xffu) ? m10 : 0.f; m11 = (cur.m1 >> 8) ? m11 : 0.f;
+    }
+    k2_products(k2_lerp(t[0]), cur.u0.x, cur.v0.x, cur.c0.x, m00 * ((in1 ? cur.c0.y : cur.c0.x) - cur.l0), m00 * (cur.c1.x - cur.cm.x),
                 o[0].x, o[1].x, o[2].x, o[3].x, o[4].x);
     k2_products(k2_lerp(t[1]), cur.u1.x, cur.v1.x, cur.c1.x, m10 * ((in1 ? cur.c1.y : cur.c1.x) - cur.l1), m10 * (cur.c2.x - cur.c0.x),
                 o[0].y, o[1].y, o[2].y, o[3].y, o[4].y);
@@ -164,7 +177,9 @@ __device__ __forceinline__ void k2_task_products(const K2Params &p, const K2In &
 // fast warps take more tiles.  Which warp computes a tile does not change its arithmetic.  `smem_cta`
 // is the CTA's dynamic shared memory, of which this warp uses slice `warp`.  Called by the stand-alone
 // kernel below and by the persistent solve kernel (of_solve.cuh).
-template <int R>
+// MK = an obstacle mask is set (p.mask and p.list are valid): a separate instantiation, so that the unmasked
+// path carries none of the mask's instructions or registers.
+template <int R, bool MK>
 __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_cta, int *tile_counter, int warp, int lane, int t_begin, int t_end)
 {
     typedef K2Geom<R> G;
@@ -184,6 +199,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
         if (lane == 0) t = atomicAdd(tile_counter, 1);
         t = __shfl_sync(0xffffffffu, t, 0) + t_begin;
         if (t >= t_end) break;
+        if (MK) t = __ldg(p.list + t);
         const int tx = t / p.tiles_y, ty = t - tx * p.tiles_y;
         const int x0 = tx * TW, y0 = ty * TH, xs = x0 - G::RL;
 
@@ -197,10 +213,10 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
             const int x = xs + 2 * cp, y = y0 + 2 * rp;
             float4 o[5];
             if (x >= 0 && x < W && y < H) {
-                const K2In in = k2_load(p, x, y);
+                const K2In in = k2_load<MK>(p, x, y);
                 K2Tap t[4];
                 k2_task_gather(p, in, x, y, t);
-                k2_task_products(p, in, x, y, t, o);
+                k2_task_products<MK>(p, in, x, y, t, o);
             } else {
 #pragma unroll
                 for (int f = 0; f < 5; ++f) o[f] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -250,7 +266,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
     }
 }
 
-template <int R>
+template <int R, bool MK>
 __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K2Params p)
 {
     extern __shared__ float4 smem4[];                          // warp slices, then 16 bytes for the tile counter
@@ -260,5 +276,5 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
     __syncthreads();
     int t_begin, t_end;
     cta_range(p.ntiles, blockIdx.x, gridDim.x, t_begin, t_end);
-    k2_phase<R>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, t_begin, t_end);
+    k2_phase<R, MK>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, t_begin, t_end);
 }

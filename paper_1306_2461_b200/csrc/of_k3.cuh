@@ -54,6 +54,7 @@ struct K3Params {
     SolveParams sp;
     int zero_uv;                     // 1 = the incoming field is identically zero and is not read (see of_k2.cuh)
     int dbg;                         // profiling switches (0 in production): 1 = no TMA/no waits, 2 = no window sum, 4 = no solve
+    MaskDesc md;                     // obstacle mask and compacted task lists of the level (all zero: none)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -149,7 +150,8 @@ template <int R> __device__ __forceinline__ int k3_cta_chunks(int t_begin, int t
 // 0..nwc-1 consume.  `gc0` = number of ring chunks this CTA has consumed in earlier passes of the same
 // kernel (keeps slot / parity bookkeeping continuous); *sm.counter must be 0 on entry (CTA-synchronised).
 // All reads of u, v go through L2 (ld.global.cg): see of_k2.cuh.
-template <int R>
+// MK = an obstacle mask is set (p.md is valid): a separate instantiation (cf. of_k2.cuh).
+template <int R, bool MK>
 __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params &p, const K3Smem &sm, int warp, int lane, int nwc,
                                          int t_begin, int t_end, uint32_t gc0)
 {
@@ -166,11 +168,9 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
     if (warp == NWC) {
         // ===================== producer: one lane walks the chunks of every segment in order
         if (lane == 0 && !(p.dbg & 1)) {
-            for (int t = t_begin; t < t_end;) {
-                const int s = t / nrb, rb0 = t - s * nrb;
-                const int ntask = min(nrb - rb0, t_end - t);
+            // one run = `ntask` consecutive tasks of strip s from row block rb0; its chunks start at ring chunk gbase
+            auto produce_run = [&](int s, int rb0, int ntask, int gbase) {
                 const int total = ntask + NC - 1;
-                const int gbase = (int)gc0 + (t - t_begin) + (s - s_first) * (NC - 1);
                 const int x0 = 64 * s, yc0 = K3_SEG * rb0 - R;          // chunk c holds rows yc0 + K3_SEG*c ...
                 for (int c = 0; c < total; ++c) {
                     const int gc = gbase + c, slot = gc % K3_RING, use = gc / K3_RING;
@@ -180,7 +180,21 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
                     mbar_expect_tx(full0 + 8 * slot, K3_CHUNK_BYTES);
                     tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + K3_SEG * c, 0, full0 + 8 * slot);
                 }
-                t += ntask;
+            };
+            if (MK) {                                                   // compacted lists: the host has cut the runs
+                const K3Cta cd = p.md.k3_cta[blockIdx.x];
+                for (int r = cd.run_b; r < cd.run_e; ++r) {
+                    const K3Run rd = p.md.k3_runs[r];
+                    const int s = rd.t0 / nrb;
+                    produce_run(s, rd.t0 - s * nrb, rd.ntask, (int)gc0 + rd.chunk_off);
+                }
+            } else {
+                for (int t = t_begin; t < t_end;) {
+                    const int s = t / nrb, rb0 = t - s * nrb;
+                    const int ntask = min(nrb - rb0, t_end - t);
+                    produce_run(s, rb0, ntask, (int)gc0 + (t - t_begin) + (s - s_first) * (NC - 1));
+                    t += ntask;
+                }
             }
         }
         __syncwarp();                                   // production done (or nothing to produce): join the consumers
@@ -192,17 +206,27 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         if (lane == 0) i = atomicAdd(counter, 1);
         i = __shfl_sync(0xffffffffu, i, 0);
         if (i >= t_end - t_begin) break;
-        const int gt = t_begin + i, s = gt / nrb, rb = gt - s * nrb;
-        const int gbase = (int)gc0 + i + (s - s_first) * (NC - 1);
+        int gt = t_begin + i, gbase;
+        if (MK) {
+            const int2 e = __ldg(p.md.k3_ent + gt);
+            gt = e.x;
+            gbase = (int)gc0 + e.y;
+        } else {
+            gbase = (int)gc0 + i + (gt / nrb - s_first) * (NC - 1);
+        }
+        const int s = gt / nrb, rb = gt - s * nrb;
         const int gx = 64 * s + 2 * lane, gy0 = K3_SEG * rb;
         const bool active = gx < W;
         // this lane's field values, issued before the waits (rows past the image re-read the last row)
         const int nrows = min(K3_SEG, H - gy0);
         const float *ui = p.u_in + (size_t)gy0 * pitch + gx, *vi = p.v_in + (size_t)gy0 * pitch + gx;
         float2 uu[K3_SEG], vv[K3_SEG];
+        unsigned mk[K3_SEG];                             // mask bytes of the lane's two columns, row by row (MK only)
 #pragma unroll
         for (int j = 0; j < K3_SEG; ++j) {
             const int jj = min(j, nrows - 1) * pitch;
+            mk[j] = 0x0101u;
+            if (MK) mk[j] = active ? __ldg(reinterpret_cast<const unsigned short *>(p.md.mask + (size_t)gy0 * pitch + gx + jj)) : 0u;
             uu[j] = (active && !p.zero_uv) ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
             vv[j] = (active && !p.zero_uv) ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
         }
@@ -248,7 +272,11 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         for (int j = 0; j < K3_SEG; ++j) {
             float2 du, dv;
             k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, trs[j], dets[j]);
-            const float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
+            float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
+            if (MK) {                                    // M3: no vector over an obstacle
+                if (!(mk[j] & 0xffu)) { un.x = 0.f; vn.x = 0.f; trs[j].x = 0.f; dets[j].x = 0.f; }
+                if (!(mk[j] >> 8)) { un.y = 0.f; vn.y = 0.f; trs[j].y = 0.f; dets[j].y = 0.f; }
+            }
             if (j < nrows) {
                 if (vec_out) {
                     *reinterpret_cast<float2 *>(uo + j * p.out_pitch) = un;
@@ -274,7 +302,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
     }
 }
 
-template <int R>
+template <int R, bool MK>
 __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const __grid_constant__ CUtensorMap tmS, const K3Params p)
 {
     extern __shared__ __align__(1024) unsigned char k3_smem_[];
@@ -283,5 +311,6 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
     __syncthreads();
     int t_begin, t_end;
     cta_range(p.ntasks, blockIdx.x, gridDim.x, t_begin, t_end);
-    k3_phase<R>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, t_begin, t_end, 0u);
+    if (MK) { t_begin = p.md.k3_cta[blockIdx.x].ent_b; t_end = p.md.k3_cta[blockIdx.x].ent_e; }
+    k3_phase<R, MK>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, t_begin, t_end, 0u);
 }

@@ -121,7 +121,8 @@ __global__ void __launch_bounds__(256) k1_pyramid_down(const T *__restrict__ src
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k4_upsample_flow(const float *__restrict__ uc, const float *__restrict__ vc,
                                                         int Wc, int Hc, int cpitch, float *__restrict__ u,
-                                                        float *__restrict__ v, int W, int H, int pitch)
+                                                        float *__restrict__ v, int W, int H, int pitch,
+                                                        const uint8_t *__restrict__ mask)   // fine-level obstacle mask or NULL (M3)
 {
     int x = blockIdx.x * 64 + (threadIdx.x & 63);
     int y = blockIdx.y * 4 + (threadIdx.x >> 6);
@@ -134,7 +135,8 @@ __global__ void __launch_bounds__(256) k4_upsample_flow(const float *__restrict_
     float ub = (1.0f - fx) * __ldg(uc + i10) + fx * __ldg(uc + i11);
     float vt = (1.0f - fx) * __ldg(vc + i00) + fx * __ldg(vc + i01);
     float vb = (1.0f - fx) * __ldg(vc + i10) + fx * __ldg(vc + i11);
-    u[(size_t)y * pitch + x] = 2.0f * ((1.0f - fy) * ut + fy * ub);
-    v[(size_t)y * pitch + x] = 2.0f * ((1.0f - fy) * vt + fy * vb);
+    const bool fluid = mask == nullptr || mask[(size_t)y * pitch + x] != 0;
+    u[(size_t)y * pitch + x] = fluid ? 2.0f * ((1.0f - fy) * ut + fy * ub) : 0.f;
+    v[(size_t)y * pitch + x] = fluid ? 2.0f * ((1.0f - fy) * vt + fy * vb) : 0.f;
 }
 

@@ -31,6 +31,7 @@ struct LevelDesc {
     int W, H, pitch;
     int k2_nseg, k2_nrp, k2_tiles_y, k2_ntiles;
     int k3_nrb, k3_ntasks;
+    MaskDesc md;                             // obstacle mask of the level (all zero: none)
 };
 
 #define SOLVE_MAX_LEVELS 12
@@ -45,6 +46,8 @@ struct SolveArgs {
     uint8_t *valid;
     float *det;
     int levels, iterations, s1, s2, out_pitch, dbg;
+    const int *zero_list;                    // level-0 K3 tasks that hold no fluid pixel (mask set): their outputs are zero-filled
+    int zero_n;
     unsigned long long *prof;                // optional timelines [ncta][SOLVE_TIMELINE_MAX] (SM clock at every phase boundary) or NULL
     WinWeights ww;
     SolveParams sp;
@@ -92,7 +95,36 @@ __device__ __forceinline__ void prof_stamp(const SolveArgs &a, int &idx)
     ++idx;
 }
 
+// M3 for the level-0 tasks no K3 pass visits: u = v = 0, valid = 0, det = 0.  One warp per task (64 x K3_SEG pixels).
+__device__ __forceinline__ void mask_zero_tasks(const int *zl, int n, int nrb, int W, int H, int pitch, float *u_out, float *v_out,
+                                                int out_pitch, uint8_t *valid, float *det, int gwarp, int nwarps, int lane)
+{
+    for (int i = gwarp; i < n; i += nwarps) {
+        const int t = __ldg(zl + i), s = t / nrb, rb = t - s * nrb;
+        for (int j = 0; j < K3_SEG; ++j) {
+            const int y = K3_SEG * rb + j;
+            for (int k = 0; k < 2; ++k) {
+                const int x = 64 * s + 32 * k + lane;
+                if (x < W && y < H) {
+                    u_out[(size_t)y * out_pitch + x] = 0.f;
+                    v_out[(size_t)y * out_pitch + x] = 0.f;
+                    valid[(size_t)y * W + x] = 0;
+                    det[(size_t)y * pitch + x] = 0.f;
+                }
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) k_mask_zero(const int *zl, int n, int nrb, int W, int H, int pitch, float *u_out, float *v_out,
+                                                   int out_pitch, uint8_t *valid, float *det)
+{
+    mask_zero_tasks(zl, n, nrb, W, H, pitch, u_out, v_out, out_pitch, valid, det, (blockIdx.x * blockDim.x + threadIdx.x) >> 5,
+                    (gridDim.x * blockDim.x) >> 5, threadIdx.x & 31);
+}
+
 // Flow hand-down (row a10, D6): u_l = 2*bilinear(u_{l+1}; x/2, y/2), grid-stride over the fine level.
+template <bool MK>
 __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDesc &C, int gtid, int nthreads)
 {
     const int W = F.W, H = F.H, Wc = C.W, Hc = C.H, cp = C.pitch, qw = (W + 3) >> 2;
@@ -115,6 +147,13 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
         vo[1] = 2.0f * (gy * (0.5f * b00 + 0.5f * b01) + fy * (0.5f * b10 + 0.5f * b11));
         vo[2] = 2.0f * (gy * (1.0f * b01 + 0.0f * b02) + fy * (1.0f * b11 + 0.0f * b12));
         vo[3] = 2.0f * (gy * (0.5f * b01 + 0.5f * b02) + fy * (0.5f * b11 + 0.5f * b12));
+        if (MK) {                                                 // M3: the field stays zero over an obstacle
+            const uchar4 m = *reinterpret_cast<const uchar4 *>(F.md.mask + y * F.pitch + x);
+            if (!m.x) { uo[0] = 0.f; vo[0] = 0.f; }
+            if (!m.y) { uo[1] = 0.f; vo[1] = 0.f; }
+            if (!m.z) { uo[2] = 0.f; vo[2] = 0.f; }
+            if (!m.w) { uo[3] = 0.f; vo[3] = 0.f; }
+        }
         float *pu = F.u + y * F.pitch + x, *pv = F.v + y * F.pitch + x;
         if (x + 3 < W) {
             *reinterpret_cast<float4 *>(pu) = make_float4(uo[0], uo[1], uo[2], uo[3]);
@@ -125,7 +164,8 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
     }
 }
 
-template <int R>
+// MK = an obstacle mask is set (of_set_mask): compacted work lists, masked products / outputs.
+template <int R, bool MK>
 __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __grid_constant__ SolveArgs a)
 {
     extern __shared__ __align__(1024) unsigned char solve_smem[];
@@ -140,24 +180,31 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
     int pi = 0;
     prof_stamp(a, pi);
     const int top = a.levels - 1;
+    if (MK && a.zero_n > 0)                                      // disjoint from everything the passes write: no barrier needed
+        mask_zero_tasks(a.zero_list, a.zero_n, a.lv[0].k3_nrb, a.lv[0].W, a.lv[0].H, a.lv[0].pitch, a.u_out, a.v_out, a.out_pitch,
+                        a.valid, a.det, cta * SOLVE_WARPS + warp, ncta * SOLVE_WARPS, lane);
     for (int l = top; l >= 0; --l) {
         const LevelDesc L = a.lv[l];
         if (l < top) {
-            upsample_phase(L, a.lv[l + 1], cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
+            upsample_phase<MK>(L, a.lv[l + 1], cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
             prof_stamp(a, pi);
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
             prof_stamp(a, pi);
         }
         int k2_b, k2_e, k3_b, k3_e;                              // this CTA's share of the level's tiles and tasks
-        cta_range(L.k2_ntiles, cta, ncta, k2_b, k2_e);
+        cta_range(MK ? L.md.k2_n : L.k2_ntiles, cta, ncta, k2_b, k2_e);
         cta_range(L.k3_ntasks, cta, ncta, k3_b, k3_e);
-        const uint32_t k3_chunks = (uint32_t)k3_cta_chunks<R>(k3_b, k3_e, L.k3_nrb);
+        uint32_t k3_chunks = (uint32_t)k3_cta_chunks<R>(k3_b, k3_e, L.k3_nrb);
+        if (MK) {                                                // mask set: the host has cut the compacted task list per CTA
+            const K3Cta cd = L.md.k3_cta[cta];
+            k3_b = cd.ent_b; k3_e = cd.ent_e; k3_chunks = (uint32_t)cd.nchunks;
+        }
         K2Params p2 = {L.pyr[a.s1], L.pyr[a.s2], L.u, L.v, a.S, a.plane, L.W, L.H, L.pitch,
-                       L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, 0, a.dbg};
+                       L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, 0, a.dbg, L.md.mask, L.md.k2_list};
         for (int it = 0; it < a.iterations; ++it) {
             // ---- K2 pass: warp + gradients + products + horizontal sums -> five planes
             p2.zero_uv = (l == top && it == 0) ? 1 : 0;            // zero initial guess at the coarsest level
-            k2_phase<R>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
+            k2_phase<R, MK>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             prof_stamp(a, pi);
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
@@ -165,9 +212,9 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             // ---- K3 pass: vertical sums + solve + update
             const bool last = (l == 0 && it == a.iterations - 1);
             K3Params p3 = {L.u, L.v, last ? a.u_out : L.u, last ? a.v_out : L.v, last ? a.valid : nullptr, last ? a.det : nullptr,
-                           L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, p2.zero_uv, a.dbg};
+                           L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, p2.zero_uv, a.dbg, L.md};
             if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async.global;" ::: "memory");
-            k3_phase<R>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            k3_phase<R, MK>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
             gc0 += k3_chunks;
             __syncthreads();
             if (threadIdx.x == 0) { sm.counter[0] = 0; sm.counter[1] = 0; }

@@ -113,6 +113,10 @@ struct of_context {
     int last_launches;
     std::string launch_err;            // first failing launch of the last enqueue ("" if none)
     std::vector<void *> allocs;
+    MaskDesc md[OF_MAX_LEVELS];         // obstacle mask + compacted work lists per level (of_set_mask); all zero = none
+    int *d_zero;                        // level-0 K3 tasks without a fluid pixel
+    int zero_n;
+    std::vector<void *> mask_allocs;
     Pipeline pipe;
 };
 
@@ -122,9 +126,12 @@ inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
 template <int R> int setup_attrs()
 {
-    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
 }
 
@@ -196,8 +203,11 @@ void launch_k2(const of_context *c, int l, const float *I1, const float *I2, boo
 {
     const Level &L = c->lv[l];
     const K2Plan &P = c->k2[l];
-    K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, P.ntiles, c->ww, zero_uv ? 1 : 0, c->dbg};
-    k2_products_hsum<R><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
+    const MaskDesc &M = c->md[l];
+    K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, M.k2_list ? M.k2_n : P.ntiles,
+                  c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list};
+    if (M.mask) k2_products_hsum<R, true><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
+    else k2_products_hsum<R, false><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
 }
 
 template <int R>
@@ -206,8 +216,9 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     const Level &L = c->lv[l];
     const K3Plan &P = c->k3[l];
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
-                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg};
-    k3_vsum_solve<R><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
+                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg, c->md[l]};
+    if (c->md[l].mask) k3_vsum_solve<R, true><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
+    else k3_vsum_solve<R, false><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
 template <int R>
@@ -218,10 +229,11 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
     a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
     a.valid = c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
+    a.zero_list = c->d_zero; a.zero_n = c->zero_n;
     a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
     a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
     void *args[] = {&a};
-    return cudaLaunchCooperativeKernel((const void *)of_solve_pair<R>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
+    return cudaLaunchCooperativeKernel(c->md[0].mask ? (const void *)of_solve_pair<R, true> : (const void *)of_solve_pair<R, false>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
                                        (size_t)K3Geom<R>::SMEM, st);
 }
 
@@ -319,7 +331,7 @@ void run_upsample(const of_context *c, int l, cudaStream_t st)   // level l+1 ->
 {
     const Level &F = c->lv[l], &Cc = c->lv[l + 1];
     dim3 grid((F.W + 63) / 64, (F.H + 3) / 4);
-    k4_upsample_flow<<<grid, 256, 0, st>>>(c->u[l + 1], c->v[l + 1], Cc.W, Cc.H, Cc.pitch, c->u[l], c->v[l], F.W, F.H, F.pitch);
+    k4_upsample_flow<<<grid, 256, 0, st>>>(c->u[l + 1], c->v[l + 1], Cc.W, Cc.H, Cc.pitch, c->u[l], c->v[l], F.W, F.H, F.pitch, c->md[l].mask);
 }
 
 void note_launch(of_context *c, const char *what, int level)
@@ -365,6 +377,11 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
         if (e != cudaSuccess && c->launch_err.empty()) c->launch_err = std::string("solve (persistent): ") + cudaGetErrorString(e);
         note_launch(c, "solve (persistent)", 0);
         return n + 1;
+    }
+    if (c->zero_n > 0) {               // mask set: outputs of the level-0 tasks no K3 pass visits (M3)
+        k_mask_zero<<<c->sms, 256, 0, st>>>(c->d_zero, c->zero_n, c->k3[0].nrb, c->W, c->H, c->lv[0].pitch, j.u_out, j.v_out, c->W, c->valid, c->det);
+        note_launch(c, "mask zero-fill", 0);
+        ++n;
     }
     for (int l = top; l >= 0; --l) {
         if (l < top) { run_upsample(c, l, st); note_launch(c, "upsample", l); ++n; }
@@ -423,6 +440,125 @@ int submit_job(of_context *c, const Job &j, cudaStream_t st)
     c->graphs.push_back({j, exec, c->stamp, n});
     CU_TRY(cudaGraphLaunch(exec, st));
     c->last_launches = n;
+    return OF_OK;
+}
+
+// Host-side construction of the mask pyramid (M4) and of the compacted work lists of one handle.
+//   K3 task (strip s, row block rb) is active iff its 64 x K3_SEG pixels hold a fluid pixel;
+//   K2 tile is active iff an active K3 task reads one of its plane rows (task rows -R .. K3_SEG-1+R);
+//   the active K3 tasks are cut into equal shares per CTA, each share into runs of consecutive tasks of
+//   one strip (a run shares ring chunks between neighbours exactly like the unmasked strip walk).
+int build_mask(of_context *c, const uint8_t *mask, int row_stride)
+{
+    for (void *p : c->mask_allocs) cudaFree(p);
+    c->mask_allocs.clear();
+    memset(c->md, 0, sizeof c->md);
+    c->d_zero = nullptr;
+    c->zero_n = 0;
+    if (!mask) return OF_OK;
+    auto upload = [&](const void *src, size_t bytes, void **dst) -> int {
+        cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
+        if (e != cudaSuccess) return fail(OF_ERR_ALLOC, "cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+        c->mask_allocs.push_back(*dst);
+        if (bytes) CU_TRY(cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice));
+        return OF_OK;
+    };
+    const int R = c->R, NC = (K3_SEG + 2 * R + K3_SEG - 1) / K3_SEG, ncta = c->sms;
+    std::vector<uint8_t> cur, nxt;
+    for (int l = 0; l < c->levels; ++l) {
+        const Level &L = c->lv[l];
+        nxt.assign((size_t)L.pitch * L.H, 0);
+        if (l == 0) {
+            for (int y = 0; y < L.H; ++y)
+                for (int x = 0; x < L.W; ++x) nxt[(size_t)y * L.pitch + x] = mask[(size_t)y * row_stride + x] ? 1 : 0;
+        } else {
+            const Level &F = c->lv[l - 1];
+            for (int Y = 0; Y < L.H; ++Y)
+                for (int X = 0; X < L.W; ++X) {
+                    int any = 0;
+                    for (int dy = 0; dy < 2; ++dy)
+                        for (int dx = 0; dx < 2; ++dx) {
+                            const int x = 2 * X + dx, y = 2 * Y + dy;
+                            if (x < F.W && y < F.H && cur[(size_t)y * F.pitch + x]) any = 1;
+                        }
+                    nxt[(size_t)Y * L.pitch + X] = (uint8_t)any;
+                }
+        }
+        cur.swap(nxt);
+        MaskDesc &M = c->md[l];
+        int rc = upload(cur.data(), cur.size(), (void **)&M.mask);
+        if (rc != OF_OK) return rc;
+        // ---- K3 tasks
+        const K3Plan &P3 = c->k3[l];
+        const int nrb = P3.nrb, nstrips = P3.ntasks / nrb;
+        std::vector<int> act, idle;
+        std::vector<uint8_t> need((size_t)nstrips * L.H, 0);
+        for (int s = 0; s < nstrips; ++s)
+            for (int rb = 0; rb < nrb; ++rb) {
+                bool any = false;
+                for (int y = K3_SEG * rb; y < std::min(K3_SEG * rb + K3_SEG, L.H) && !any; ++y)
+                    for (int x = 64 * s; x < std::min(64 * s + 64, L.W); ++x)
+                        if (cur[(size_t)y * L.pitch + x]) { any = true; break; }
+                if (!any) { idle.push_back(s * nrb + rb); continue; }
+                act.push_back(s * nrb + rb);
+                for (int y = std::max(0, K3_SEG * rb - R); y <= std::min(L.H - 1, K3_SEG * rb + K3_SEG - 1 + R); ++y) need[(size_t)s * L.H + y] = 1;
+            }
+        std::vector<int2> ent(act.size());
+        std::vector<K3Run> runs;
+        std::vector<K3Cta> ctas(ncta);
+        for (int cta = 0; cta < ncta; ++cta) {
+            int b, e;
+            cta_range((int)act.size(), cta, ncta, b, e);
+            K3Cta cd = {b, e, (int)runs.size(), 0, 0, 0, 0, 0};
+            int chunks = 0;
+            for (int i = b; i < e;) {
+                int n = 1;
+                while (i + n < e && act[i + n] == act[i] + n && act[i + n] / nrb == act[i] / nrb) ++n;
+                runs.push_back({act[i], n, chunks, 0});
+                for (int k = 0; k < n; ++k) ent[i + k] = make_int2(act[i + k], chunks + k);
+                chunks += n + NC - 1;
+                i += n;
+            }
+            cd.run_e = (int)runs.size();
+            cd.nchunks = chunks;
+            ctas[cta] = cd;
+        }
+        M.k3_n = (int)act.size();
+        if ((rc = upload(ent.data(), ent.size() * sizeof(int2), (void **)&M.k3_ent)) != OF_OK) return rc;
+        if ((rc = upload(runs.data(), runs.size() * sizeof(K3Run), (void **)&M.k3_runs)) != OF_OK) return rc;
+        if ((rc = upload(ctas.data(), ctas.size() * sizeof(K3Cta), (void **)&M.k3_cta)) != OF_OK) return rc;
+        if (l == 0) {
+            c->zero_n = (int)idle.size();
+            if ((rc = upload(idle.data(), idle.size() * sizeof(int), (void **)&c->d_zero)) != OF_OK) return rc;
+        }
+        // ---- K2 tiles
+        const K2Plan &P2 = c->k2[l];
+        const int TW = 8 * P2.nseg, TH = 2 * P2.nrp, tiles_x = P2.ntiles / P2.tiles_y;
+        std::vector<int> tiles;
+        for (int tx = 0; tx < tiles_x; ++tx)
+            for (int ty = 0; ty < P2.tiles_y; ++ty) {
+                bool any = false;
+                const int s0 = (tx * TW) / 64, s1 = std::min(nstrips - 1, (tx * TW + TW - 1) / 64);
+                for (int sidx = s0; sidx <= s1 && !any; ++sidx)
+                    for (int y = ty * TH; y < std::min(ty * TH + TH, L.H); ++y)
+                        if (need[(size_t)sidx * L.H + y]) { any = true; break; }
+                if (any) tiles.push_back(tx * P2.tiles_y + ty);
+            }
+        M.k2_n = (int)tiles.size();
+        if ((rc = upload(tiles.data(), tiles.size() * sizeof(int), (void **)&M.k2_list)) != OF_OK) return rc;
+        if (getenv("OF_DEBUG"))
+            fprintf(stderr, "[optflow] mask level %d: K2 tiles %d of %d, K3 tasks %d of %d (%zu runs)\n", l, M.k2_n, P2.ntiles, M.k3_n, P3.ntasks, runs.size());
+    }
+    return OF_OK;
+}
+
+int upload_level_descs(of_context *c)
+{
+    LevelDesc hl[OF_MAX_LEVELS];
+    for (int l = 0; l < c->levels; ++l)
+        hl[l] = {{c->pyr[0][l], c->pyr[1][l]}, c->u[l], c->v[l], c->lv[l].W, c->lv[l].H, c->lv[l].pitch,
+                 c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks, c->md[l]};
+    CU_TRY(cudaMemcpy(c->d_lv, hl, sizeof(LevelDesc) * c->levels, cudaMemcpyHostToDevice));
     return OF_OK;
 }
 
@@ -570,11 +706,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_post, 256);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_prof, sizeof(unsigned long long) * OF_TIMELINE_MAX * c->sms);
         if (rc == OF_OK) {
-            LevelDesc hl[OF_MAX_LEVELS];
-            for (int l = 0; l < levels; ++l)
-                hl[l] = {{c->pyr[0][l], c->pyr[1][l]}, c->u[l], c->v[l], lv[l].W, lv[l].H, lv[l].pitch,
-                         c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks};
-            cudaMemcpy(c->d_lv, hl, sizeof(LevelDesc) * levels, cudaMemcpyHostToDevice);
+            rc = upload_level_descs(c);
             cudaMemcpy(c->d_tm, c->tmS, sizeof(CUtensorMap) * levels, cudaMemcpyHostToDevice);
             cudaMemset(c->d_gbar, 0, 256);
             if (cudaDeviceSynchronize() != cudaSuccess) rc = fail(OF_ERR_CUDA, "descriptor upload failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -600,6 +732,7 @@ void of_destroy(of_handle h)
     cudaDeviceSynchronize();
     drop_graphs(h);
     for (void *p : h->allocs) cudaFree(p);
+    for (void *p : h->mask_allocs) cudaFree(p);
     delete h;
 }
 
@@ -638,6 +771,27 @@ int of_set_equalisation(of_handle h, int radius)
     }
     h->eq_radius = radius;
     drop_graphs(h);
+    return OF_OK;
+}
+
+int of_set_mask(of_handle h, const uint8_t *mask_host, int row_stride)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    if (mask_host && row_stride < h->W) return fail(OF_ERR_INVALID_ARG, "row_stride %d is smaller than the width %d", row_stride, h->W);
+    CU_TRY(cudaSetDevice(h->device));
+    CU_TRY(cudaDeviceSynchronize());                   // set-up call: nothing of this handle may be in flight
+    drop_graphs(h);
+    int rc = build_mask(h, mask_host, row_stride);
+    if (rc != OF_OK) { std::string keep = g_err; build_mask(h, nullptr, 0); upload_level_descs(h); g_err = keep; return rc; }
+    // tasks that no pass visits must read as "no vector" for ever: the level fields start from zero (M3)
+    for (int l = 0; l < h->levels; ++l) {
+        const size_t bytes = sizeof(float) * (size_t)h->lv[l].pitch * h->lv[l].H;
+        CU_TRY(cudaMemset(h->u[l], 0, bytes));
+        CU_TRY(cudaMemset(h->v[l], 0, bytes));
+    }
+    rc = upload_level_descs(h);
+    if (rc != OF_OK) return rc;
+    CU_TRY(cudaDeviceSynchronize());
     return OF_OK;
 }
 
@@ -789,7 +943,7 @@ int of_upsample_flow(const float *uc, const float *vc, int wc, int hc, float *u,
     if (!uc || !vc || !u || !v || wc < 1 || hc < 1 || width < 1 || height < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
     if (wc != (width + 1) / 2 || hc != (height + 1) / 2) return fail(OF_ERR_INVALID_ARG, "coarse size must be ((W+1)/2,(H+1)/2)");
     dim3 grid((width + 63) / 64, (height + 3) / 4);
-    k4_upsample_flow<<<grid, 256, 0, (cudaStream_t)stream>>>(uc, vc, wc, hc, wc, u, v, width, height, width);
+    k4_upsample_flow<<<grid, 256, 0, (cudaStream_t)stream>>>(uc, vc, wc, hc, wc, u, v, width, height, width, nullptr);
     CU_TRY(cudaGetLastError());
     return OF_OK;
 }

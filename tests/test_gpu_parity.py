@@ -428,3 +428,89 @@ def test_bubble_surface_counts_match_oracle_exactly(torch, B, oracle):
         assert tuple(cnt.cpu().tolist()) == oracle.bubble_counts(fields[2].cpu().numpy(), float(T), mh)
         assert tuple(cnt_all.cpu().tolist()) == oracle.bubble_counts(fields[2].cpu().numpy(), float(T))
         assert 0 < cnt[0] < cnt[1] <= W * H
+
+
+# ---------------------------------------------------------------------------- NEXT item f4: obstacle masks
+def gpu_solve_masked(torch, B, c, mask, persistent=True, graph=True, then_clear=False):
+    with B.OpticalFlow(c.width, c.height, c.levels, c.window_radius, c.iterations, c.window_type) as of:
+        of.set_graph(graph)
+        of.set_persistent(persistent)
+        of.set_mask(mask)
+        d1 = torch.from_numpy(c.I1.view(np.int16) if c.I1.dtype == np.uint16 else c.I1).cuda()
+        d2 = torch.from_numpy(c.I2.view(np.int16) if c.I2.dtype == np.uint16 else c.I2).cuda()
+        s = torch.cuda.Stream()
+        out = []
+        with torch.cuda.stream(s):
+            for rep in range(2):                       # twice: the second solve starts from the fields the first one left
+                u = torch.full((c.height, c.width), 7.0, dtype=torch.float32, device="cuda")   # stale values must be overwritten
+                v = torch.full((c.height, c.width), -7.0, dtype=torch.float32, device="cuda")
+                of.compute(d1, d2, u, v)
+                out.append((u.cpu().numpy(), v.cpu().numpy(), of.validity().cpu().numpy()))
+            if then_clear:
+                of.set_mask(None)
+                u, v = of.compute(d1, d2)
+                out.append((u.cpu().numpy(), v.cpu().numpy(), of.validity().cpu().numpy()))
+        s.synchronize()
+        return out
+
+
+def _blob_mask(H, W):
+    m = np.ones((H, W), dtype=np.uint8)
+    m[H // 4:H // 2, W // 8:W // 2] = 0
+    m[:, :3] = 0
+    m[(3 * H) // 4, (3 * W) // 4] = 0
+    return m
+
+
+@pytest.mark.parametrize("case,maskfn", [
+    (lambda: syn.config1(), _blob_mask),
+    (lambda: syn.config2(203, 157), _blob_mask),
+    (lambda: syn.config3(320, 256), lambda H, W: syn.mask_backward_step(W, H)),
+    (lambda: syn.config4(256, 192), _blob_mask),
+    (lambda: syn.config3(), lambda H, W: syn.mask_backward_step(W, H)),
+], ids=["config1", "config2-ragged", "config3-small-step", "config4-small-u16", "config3-1280x1024-step"])
+def test_masked_solve_matches_oracle(torch, B, oracle, case, maskfn):
+    """Readings M1-M5: parity on the fluid pixels, exactly no vector over the obstacle, identical validity;
+    the persistent kernel and the per-kernel launches agree bit for bit; a repeat gives the same bits."""
+    c = case()
+    mask = maskfn(c.height, c.width)
+    ref = oracle.solve(c.I1, c.I2, c.levels, c.window_radius, c.iterations, c.window_type, mask=mask)
+    runs = gpu_solve_masked(torch, B, c, mask)
+    u, v, m = runs[0]
+    st = assert_parity(u, v, m, ref, c.name + "+mask")
+    print(c.name, "masked", st)
+    assert np.all(u[mask == 0] == 0.0) and np.all(v[mask == 0] == 0.0) and np.all(m[mask == 0] == 0)
+    assert np.array_equal(runs[1][0], u) and np.array_equal(runs[1][1], v) and np.array_equal(runs[1][2], m)
+    u2, v2, m2 = gpu_solve_masked(torch, B, c, mask, persistent=False, graph=False)[0]
+    assert np.array_equal(u2, u) and np.array_equal(v2, v) and np.array_equal(m2, m)
+
+
+def test_mask_of_ones_zeros_and_removal(torch, B):
+    c = syn.config3(320, 256)
+    plain = gpu_solve(torch, B, c.I1, c.I2, c.levels, c.window_radius, c.iterations, c.window_type)
+    ones = gpu_solve_masked(torch, B, c, np.ones((c.height, c.width), np.uint8))[0]
+    assert np.array_equal(ones[0], plain[0]) and np.array_equal(ones[1], plain[1]) and np.array_equal(ones[2], plain[2])
+    runs = gpu_solve_masked(torch, B, c, np.zeros((c.height, c.width), np.uint8), then_clear=True)
+    assert not runs[0][0].any() and not runs[0][1].any() and not runs[0][2].any()
+    assert np.array_equal(runs[2][0], plain[0]) and np.array_equal(runs[2][1], plain[1]) and np.array_equal(runs[2][2], plain[2])
+
+
+def test_mask_skips_work(torch, B):
+    """The point of the mask (PAPER.md:175 'higher speeds'): the solve of a half-masked frame is faster."""
+    c = syn.config3()
+    mask = np.ones((c.height, c.width), np.uint8)
+    mask[:, c.width // 2:] = 0
+    with B.OpticalFlow(c.width, c.height, c.levels, c.window_radius, c.iterations, c.window_type) as of:
+        d1, d2 = torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()
+        of.compute(d1, d2)
+        def timed():
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            of.run_solve(5)
+            a.record(); of.run_solve(20); b.record(); b.synchronize()
+            return a.elapsed_time(b) / 20
+        t_full = timed()
+        of.set_mask(mask)
+        of.compute(d1, d2)
+        t_half = timed()
+    print("solve ms: unmasked %.3f, right half masked %.3f" % (t_full, t_half))
+    assert t_half < 0.9 * t_full

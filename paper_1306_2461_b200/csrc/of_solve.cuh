@@ -133,6 +133,8 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
         const int x0 = x >> 1, x1 = min(x0 + 1, Wc - 1), x2 = min(x0 + 2, Wc - 1), y0 = y >> 1, y1 = min(y0 + 1, Hc - 1);
         const float fy = (y & 1) * 0.5f, gy = 1.0f - fy;
         const float *ur0 = C.u + y0 * cp, *ur1 = C.u + y1 * cp, *vr0 = C.v + y0 * cp, *vr1 = C.v + y1 * cp;
+        uchar4 m = make_uchar4(1, 1, 1, 1);
+        if (MK) m = __ldg(reinterpret_cast<const uchar4 *>(F.md.mask + y * F.pitch + x));   // issued with the field loads
         const float a00 = __ldcg(ur0 + x0), a01 = __ldcg(ur0 + x1), a02 = __ldcg(ur0 + x2);
         const float a10 = __ldcg(ur1 + x0), a11 = __ldcg(ur1 + x1), a12 = __ldcg(ur1 + x2);
         const float b00 = __ldcg(vr0 + x0), b01 = __ldcg(vr0 + x1), b02 = __ldcg(vr0 + x2);
@@ -148,7 +150,6 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
         vo[2] = 2.0f * (gy * (1.0f * b01 + 0.0f * b02) + fy * (1.0f * b11 + 0.0f * b12));
         vo[3] = 2.0f * (gy * (0.5f * b01 + 0.5f * b02) + fy * (0.5f * b11 + 0.5f * b12));
         if (MK) {                                                 // M3: the field stays zero over an obstacle
-            const uchar4 m = *reinterpret_cast<const uchar4 *>(F.md.mask + y * F.pitch + x);
             if (!m.x) { uo[0] = 0.f; vo[0] = 0.f; }
             if (!m.y) { uo[1] = 0.f; vo[1] = 0.f; }
             if (!m.z) { uo[2] = 0.f; vo[2] = 0.f; }

@@ -138,7 +138,7 @@ template <int R> int setup_attrs()
 // K2: warp tiles of (8*nseg) x (2*nrp) outputs; every CTA owns an equal range of tiles and its
 // SOLVE_WARPS warps pull from it.  The model only ranks candidates by the serial latency of a CTA's pass
 // (coarse levels: one-round tiles with field-parallel sums; fine levels: fewer, wider tiles).
-template <int R> K2Plan plan_k2(int W, int H, int sms)
+template <int R> K2Plan plan_k2(int W, int H, int sms, double active = 1.0)   // active = share of the tiles a mask leaves
 {
     typedef K2Geom<R> G;
     K2Plan best = {};
@@ -164,7 +164,7 @@ template <int R> K2Plan plan_k2(int W, int H, int sms)
             // Serial latency of a CTA's pass, in SM cycles, fitted to the in-kernel timeline (profiles/
             // r1_experiments.md): a tile costs 1850 + 1300 per product round + (550 + 400 x warps sharing a
             // sub-partition's FMA pipe) per serial field sum; a CTA runs its tiles in waves of SOLVE_WARPS.
-            const int tiles_cta = (ntiles + sms - 1) / sms;
+            const int tiles_cta = ((int)std::ceil(ntiles * active) + sms - 1) / sms;
             double cost = 0.0;
             for (int left = tiles_cta; left > 0; left -= SOLVE_WARPS) {
                 const int conc = std::min(left, SOLVE_WARPS);
@@ -455,7 +455,10 @@ int build_mask(of_context *c, const uint8_t *mask, int row_stride)
     memset(c->md, 0, sizeof c->md);
     c->d_zero = nullptr;
     c->zero_n = 0;
-    if (!mask) return OF_OK;
+    if (!mask) {
+        for (int l = 0; l < c->levels; ++l) { DISPATCH_R(c->R, c->k2[l] = plan_k2<R>(c->lv[l].W, c->lv[l].H, c->sms)); }
+        return OF_OK;
+    }
     auto upload = [&](const void *src, size_t bytes, void **dst) -> int {
         cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
         if (e != cudaSuccess) return fail(OF_ERR_ALLOC, "cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
@@ -531,7 +534,13 @@ int build_mask(of_context *c, const uint8_t *mask, int row_stride)
             c->zero_n = (int)idle.size();
             if ((rc = upload(idle.data(), idle.size() * sizeof(int), (void **)&c->d_zero)) != OF_OK) return rc;
         }
-        // ---- K2 tiles
+        // ---- K2 tiles (geometry re-planned for the share of the level that is left)
+        {
+            size_t cnt = 0;
+            for (uint8_t b : need) cnt += b;
+            const double share = std::max(0.02, (double)cnt / (double)std::max<size_t>(need.size(), 1));
+            DISPATCH_R(c->R, c->k2[l] = plan_k2<R>(L.W, L.H, c->sms, share));
+        }
         const K2Plan &P2 = c->k2[l];
         const int TW = 8 * P2.nseg, TH = 2 * P2.nrp, tiles_x = P2.ntiles / P2.tiles_y;
         std::vector<int> tiles;

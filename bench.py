@@ -310,7 +310,7 @@ def run_ours(args):
                     "d2h_bytes_per_step": 8 * px, "steps": e2e_steps,
                     "api": "of_stream_open(PAIRS, host results) / acquire+fill / submit / result", "checksum": checksum},
             "gpu_launches": launches,
-            "roofline": {"bound": "hbm", "kernel": "of_solve_pair<12> (persistent: K2 pass + K3 pass + hand-down, all levels and iterations)",
+            "roofline": {"bound": "hbm", "kernel": "of_solve_pair<12, false> (persistent: K2 pass + K3 pass + hand-down, all levels and iterations)",
                          "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                          "traffic": NCU_DRAM_BYTES_PER_SOLVE, "traffic_source": "profiles/r1_persistent_solve.md (ncu --set full, dram read + write of one launch; the 47 MB of planes are L2 resident)",
                          "peak_source": peak_src, "bytes_per_launch": solve_bytes,

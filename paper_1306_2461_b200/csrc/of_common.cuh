@@ -33,4 +33,6 @@ struct MaskDesc {                                         // all zero when no ma
     const K3Run *k3_runs;
     const K3Cta *k3_cta;                                  // [number of CTAs]
     int k2_n, k3_n;
+    const int *zero_list;                                 // level 0 only: K3 tasks without a fluid pixel (their outputs are zero-filled)
+    int zero_n, pad;
 };

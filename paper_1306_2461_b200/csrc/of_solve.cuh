@@ -31,7 +31,6 @@ struct LevelDesc {
     int W, H, pitch;
     int k2_nseg, k2_nrp, k2_tiles_y, k2_ntiles;
     int k3_nrb, k3_ntasks;
-    MaskDesc md;                             // obstacle mask of the level (all zero: none)
 };
 
 #define SOLVE_MAX_LEVELS 12
@@ -46,11 +45,11 @@ struct SolveArgs {
     uint8_t *valid;
     float *det;
     int levels, iterations, s1, s2, out_pitch, dbg;
-    const int *zero_list;                    // level-0 K3 tasks that hold no fluid pixel (mask set): their outputs are zero-filled
-    int zero_n;
     unsigned long long *prof;                // optional timelines [ncta][SOLVE_TIMELINE_MAX] (SM clock at every phase boundary) or NULL
     WinWeights ww;
     SolveParams sp;
+    const MaskDesc *md;                      // device array [levels]: obstacle masks and work lists (read by the MK kernel only;
+                                             // last, so that every other field keeps its place in the parameter bank)
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
@@ -125,7 +124,7 @@ __global__ void __launch_bounds__(256) k_mask_zero(const int *zl, int n, int nrb
 
 // Flow hand-down (row a10, D6): u_l = 2*bilinear(u_{l+1}; x/2, y/2), grid-stride over the fine level.
 template <bool MK>
-__device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDesc &C, int gtid, int nthreads)
+__device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDesc &C, const uint8_t *fmask, int gtid, int nthreads)
 {
     const int W = F.W, H = F.H, Wc = C.W, Hc = C.H, cp = C.pitch, qw = (W + 3) >> 2;
     for (int i = gtid; i < qw * H; i += nthreads) {              // four adjacent fine pixels per thread
@@ -134,7 +133,7 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
         const float fy = (y & 1) * 0.5f, gy = 1.0f - fy;
         const float *ur0 = C.u + y0 * cp, *ur1 = C.u + y1 * cp, *vr0 = C.v + y0 * cp, *vr1 = C.v + y1 * cp;
         uchar4 m = make_uchar4(1, 1, 1, 1);
-        if (MK) m = __ldg(reinterpret_cast<const uchar4 *>(F.md.mask + y * F.pitch + x));   // issued with the field loads
+        if (MK) m = __ldg(reinterpret_cast<const uchar4 *>(fmask + y * F.pitch + x));   // issued with the field loads
         const float a00 = __ldcg(ur0 + x0), a01 = __ldcg(ur0 + x1), a02 = __ldcg(ur0 + x2);
         const float a10 = __ldcg(ur1 + x0), a11 = __ldcg(ur1 + x1), a12 = __ldcg(ur1 + x2);
         const float b00 = __ldcg(vr0 + x0), b01 = __ldcg(vr0 + x1), b02 = __ldcg(vr0 + x2);
@@ -181,27 +180,29 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
     int pi = 0;
     prof_stamp(a, pi);
     const int top = a.levels - 1;
-    if (MK && a.zero_n > 0)                                      // disjoint from everything the passes write: no barrier needed
-        mask_zero_tasks(a.zero_list, a.zero_n, a.lv[0].k3_nrb, a.lv[0].W, a.lv[0].H, a.lv[0].pitch, a.u_out, a.v_out, a.out_pitch,
+    if (MK && a.md[0].zero_n > 0)                                // disjoint from everything the passes write: no barrier needed
+        mask_zero_tasks(a.md[0].zero_list, a.md[0].zero_n, a.lv[0].k3_nrb, a.lv[0].W, a.lv[0].H, a.lv[0].pitch, a.u_out, a.v_out, a.out_pitch,
                         a.valid, a.det, cta * SOLVE_WARPS + warp, ncta * SOLVE_WARPS, lane);
     for (int l = top; l >= 0; --l) {
         const LevelDesc L = a.lv[l];
+        MaskDesc M = {};
+        if (MK) M = a.md[l];
         if (l < top) {
-            upsample_phase<MK>(L, a.lv[l + 1], cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
+            upsample_phase<MK>(L, a.lv[l + 1], M.mask, cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
             prof_stamp(a, pi);
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
             prof_stamp(a, pi);
         }
         int k2_b, k2_e, k3_b, k3_e;                              // this CTA's share of the level's tiles and tasks
-        cta_range(MK ? L.md.k2_n : L.k2_ntiles, cta, ncta, k2_b, k2_e);
+        cta_range(MK ? M.k2_n : L.k2_ntiles, cta, ncta, k2_b, k2_e);
         cta_range(L.k3_ntasks, cta, ncta, k3_b, k3_e);
         uint32_t k3_chunks = (uint32_t)k3_cta_chunks<R>(k3_b, k3_e, L.k3_nrb);
         if (MK) {                                                // mask set: the host has cut the compacted task list per CTA
-            const K3Cta cd = L.md.k3_cta[cta];
+            const K3Cta cd = M.k3_cta[cta];
             k3_b = cd.ent_b; k3_e = cd.ent_e; k3_chunks = (uint32_t)cd.nchunks;
         }
         K2Params p2 = {L.pyr[a.s1], L.pyr[a.s2], L.u, L.v, a.S, a.plane, L.W, L.H, L.pitch,
-                       L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, 0, a.dbg, L.md.mask, L.md.k2_list};
+                       L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, 0, a.dbg, M.mask, M.k2_list};
         for (int it = 0; it < a.iterations; ++it) {
             // ---- K2 pass: warp + gradients + products + horizontal sums -> five planes
             p2.zero_uv = (l == top && it == 0) ? 1 : 0;            // zero initial guess at the coarsest level
@@ -213,7 +214,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             // ---- K3 pass: vertical sums + solve + update
             const bool last = (l == 0 && it == a.iterations - 1);
             K3Params p3 = {L.u, L.v, last ? a.u_out : L.u, last ? a.v_out : L.v, last ? a.valid : nullptr, last ? a.det : nullptr,
-                           L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, p2.zero_uv, a.dbg, L.md};
+                           L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, p2.zero_uv, a.dbg, M};
             if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async.global;" ::: "memory");
             k3_phase<R, MK>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
             gc0 += k3_chunks;

@@ -101,6 +101,7 @@ struct of_context {
     K3Plan k3[OF_MAX_LEVELS];
     CUtensorMap tmS[OF_MAX_LEVELS];     // the five summed planes of a level as one (x, y, field) tensor
     LevelDesc *d_lv;                    // device copies for the persistent solve kernel
+    MaskDesc *d_md;
     CUtensorMap *d_tm;
     unsigned *d_gbar;
     unsigned *d_post;                   // scratch of the post-processing reductions (min/max words)
@@ -229,7 +230,7 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
     a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
     a.valid = c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
-    a.zero_list = c->d_zero; a.zero_n = c->zero_n;
+    a.md = c->d_md;
     a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
     a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
     void *args[] = {&a};
@@ -533,6 +534,8 @@ int build_mask(of_context *c, const uint8_t *mask, int row_stride)
         if (l == 0) {
             c->zero_n = (int)idle.size();
             if ((rc = upload(idle.data(), idle.size() * sizeof(int), (void **)&c->d_zero)) != OF_OK) return rc;
+            M.zero_list = c->d_zero;
+            M.zero_n = c->zero_n;
         }
         // ---- K2 tiles (geometry re-planned for the share of the level that is left)
         {
@@ -566,8 +569,9 @@ int upload_level_descs(of_context *c)
     LevelDesc hl[OF_MAX_LEVELS];
     for (int l = 0; l < c->levels; ++l)
         hl[l] = {{c->pyr[0][l], c->pyr[1][l]}, c->u[l], c->v[l], c->lv[l].W, c->lv[l].H, c->lv[l].pitch,
-                 c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks, c->md[l]};
+                 c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks};
     CU_TRY(cudaMemcpy(c->d_lv, hl, sizeof(LevelDesc) * c->levels, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(c->d_md, c->md, sizeof(MaskDesc) * c->levels, cudaMemcpyHostToDevice));
     return OF_OK;
 }
 
@@ -710,6 +714,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         for (int l = 0; l < levels; ++l) { DISPATCH_R(window_radius, plan_level<R>(c, l)); }
         rc = encode_tensor_maps(c);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_lv, sizeof(LevelDesc) * levels);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_md, sizeof(MaskDesc) * OF_MAX_LEVELS);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_tm, sizeof(CUtensorMap) * levels);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_gbar, 256);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_post, 256);

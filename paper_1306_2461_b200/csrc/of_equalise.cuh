@@ -17,17 +17,22 @@ template <typename T> struct EqAcc { typedef unsigned int S1; typedef unsigned l
 template <> struct EqAcc<uint8_t> { typedef unsigned int S1; typedef unsigned int S2; };       // 33^2 * 255^2 < 2^32
 template <> struct EqAcc<float> { typedef double S1; typedef double S2; };
 
+#define EQ_HS (EQ_TW + 1)                                   // row stride of the row-sum arrays (odd: spreads the banks)
+
 __host__ __device__ inline size_t eq_smem_bytes(int r, size_t elem)
 {
     const size_t pw = EQ_TW + 2 * r, ph = EQ_TH + 2 * r;
-    return ph * pw * elem + ph * EQ_TW * (sizeof(unsigned long long) + sizeof(double));   // patch + row sums (upper bound)
+    const size_t s1 = elem == 4 ? 8 : 4, s2 = elem == 1 ? 4 : 8;           // sizeof(EqAcc<T>::S1), sizeof(EqAcc<T>::S2)
+    return (ph * pw * elem + 15) / 16 * 16 + ph * EQ_HS * (s1 + s2) + 16;  // patch + row sums
 }
 
-template <typename T>
+// RT = the radius as a compile-time constant (the paper's 5: every loop unrolls) or 0 = run-time radius r_arg.
+template <typename T, int RT = 0>
 __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, const T *__restrict__ srcB,
                                                    float *__restrict__ dstA, float *__restrict__ dstB,
-                                                   int W, int H, int pitch, int r)
+                                                   int W, int H, int pitch, int r_arg)
 {
+    const int r = RT ? RT : r_arg;
     typedef typename EqAcc<T>::S1 S1;
     typedef typename EqAcc<T>::S2 S2;
     const T *__restrict__ src = blockIdx.z ? srcB : srcA;
@@ -35,14 +40,18 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
     if (src == nullptr) return;
     extern __shared__ __align__(16) unsigned char eq_smem[];
     const int pw = EQ_TW + 2 * r, ph = EQ_TH + 2 * r;
-    S2 *h2 = reinterpret_cast<S2 *>(eq_smem);                         // [ph][EQ_TW] row sums of I^2
-    S1 *h1 = reinterpret_cast<S1 *>(h2 + (size_t)ph * EQ_TW);         // [ph][EQ_TW] row sums of I
-    T *patch = reinterpret_cast<T *>(h1 + (size_t)ph * EQ_TW);        // [ph][pw] raw values, 0 outside the image
+    S2 *h2 = reinterpret_cast<S2 *>(eq_smem);                         // [ph][EQ_HS] row sums of I^2
+    S1 *h1 = reinterpret_cast<S1 *>(h2 + (size_t)ph * EQ_HS + (sizeof(S2) == 4 ? (ph & 1) : 0));   // [ph][EQ_HS] row sums of I (8-byte aligned)
+    T *patch = reinterpret_cast<T *>(h1 + (size_t)ph * EQ_HS);        // [ph][pw] raw values, 0 outside the image
     const int x0 = blockIdx.x * EQ_TW, y0 = blockIdx.y * EQ_TH;
-    for (int i = threadIdx.x; i < ph * pw; i += 256) {
-        const int py = i / pw, px = i - py * pw;
-        const int gx = x0 - r + px, gy = y0 - r + py;
-        patch[i] = (gx >= 0 && gx < W && gy >= 0 && gy < H) ? src[(size_t)gy * W + gx] : T(0);
+    for (int py = threadIdx.x >> 5; py < ph; py += 8) {               // a warp per patch row: coalesced, no divisions
+        const int gy = y0 - r + py;
+        const bool row_ok = gy >= 0 && gy < H;
+        const T *srow = src + (size_t)gy * W;
+        for (int px = threadIdx.x & 31; px < pw; px += 32) {
+            const int gx = x0 - r + px;
+            patch[py * pw + px] = (row_ok && gx >= 0 && gx < W) ? __ldg(srow + gx) : T(0);
+        }
     }
     __syncthreads();
     // pass 1, along rows: one thread per (patch row, 8 adjacent outputs).  Integer frames slide the box
@@ -52,13 +61,15 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
         const T *p = patch + py * pw + x8;
         S1 s = 0;
         S2 s2 = 0;
+#pragma unroll
         for (int d = 0; d <= 2 * r; ++d) {
             const S1 v = (S1)p[d];
             s += v;
             s2 += (S2)v * (S2)v;
         }
-        h1[py * EQ_TW + x8] = s;
-        h2[py * EQ_TW + x8] = s2;
+        h1[py * EQ_HS + x8] = s;
+        h2[py * EQ_HS + x8] = s2;
+#pragma unroll
         for (int k = 1; k < 8; ++k) {
             if (sizeof(T) == 4) {
                 s = 0;
@@ -73,8 +84,8 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
                 s += a - b;
                 s2 += (S2)a * (S2)a - (S2)b * (S2)b;
             }
-            h1[py * EQ_TW + x8 + k] = s;
-            h2[py * EQ_TW + x8 + k] = s2;
+            h1[py * EQ_HS + x8 + k] = s;
+            h2[py * EQ_HS + x8 + k] = s2;
         }
     }
     __syncthreads();
@@ -84,18 +95,20 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
         const int gx = x0 + x;
         S1 s = 0;
         S2 s2 = 0;
+#pragma unroll
         for (int k = 0; k < 8; ++k) {
             const int y = y8 + k, gy = y0 + y;
             if (k == 0 || sizeof(T) == 4) {
                 s = 0;
                 s2 = 0;
+#pragma unroll
                 for (int d = 0; d <= 2 * r; ++d) {
-                    s += h1[(y + d) * EQ_TW + x];
-                    s2 += h2[(y + d) * EQ_TW + x];
+                    s += h1[(y + d) * EQ_HS + x];
+                    s2 += h2[(y + d) * EQ_HS + x];
                 }
             } else {
-                s += h1[(y + 2 * r) * EQ_TW + x] - h1[(y - 1) * EQ_TW + x];
-                s2 += h2[(y + 2 * r) * EQ_TW + x] - h2[(y - 1) * EQ_TW + x];
+                s += h1[(y + 2 * r) * EQ_HS + x] - h1[(y - 1) * EQ_HS + x];
+                s2 += h2[(y + 2 * r) * EQ_HS + x] - h2[(y - 1) * EQ_HS + x];
             }
             if (gx >= W || gy >= H) continue;
             const int n = (min(gx + r, W - 1) - max(gx - r, 0) + 1) * (min(gy + r, H - 1) - max(gy - r, 0) + 1);
@@ -107,7 +120,7 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
             } else {                                                       // integer frames: exact numerators
                 const long long num = (long long)n * (long long)s2 - (long long)s * (long long)s;
                 const long long top = (long long)c * n - (long long)s;
-                out = num > 0 ? (float)top / sqrtf((float)num) : 0.f;
+                out = num > 0 ? (float)top * rsqrtf((float)num) : 0.f;      // MUFU.RSQ, <= 2 ulp; the zero decision is exact
             }
             dst[(size_t)gy * pitch + gx] = out;
         }

@@ -291,7 +291,11 @@ void run_convert(const of_context *c, int dtype, const void *a, const void *b, f
     if (c->eq_radius > 0) {                                            // eq. 2 fused with the conversion
         const int r = c->eq_radius;
         dim3 grid((L.W + EQ_TW - 1) / EQ_TW, (L.H + EQ_TH - 1) / EQ_TH, b ? 2 : 1);
-        if (dtype == OF_DTYPE_U8)
+        if (dtype == OF_DTYPE_U8 && r == 5)                               // the paper's radius: unrolled instantiation
+            k0_equalise<uint8_t, 5><<<grid, 256, eq_smem_bytes(r, 1), st>>>((const uint8_t *)a, (const uint8_t *)b, da, db, L.W, L.H, L.pitch, r);
+        else if (dtype == OF_DTYPE_U16 && r == 5)
+            k0_equalise<uint16_t, 5><<<grid, 256, eq_smem_bytes(r, 2), st>>>((const uint16_t *)a, (const uint16_t *)b, da, db, L.W, L.H, L.pitch, r);
+        else if (dtype == OF_DTYPE_U8)
             k0_equalise<uint8_t><<<grid, 256, eq_smem_bytes(r, 1), st>>>((const uint8_t *)a, (const uint8_t *)b, da, db, L.W, L.H, L.pitch, r);
         else if (dtype == OF_DTYPE_U16)
             k0_equalise<uint16_t><<<grid, 256, eq_smem_bytes(r, 2), st>>>((const uint16_t *)a, (const uint16_t *)b, da, db, L.W, L.H, L.pitch, r);
@@ -782,6 +786,8 @@ int of_set_equalisation(of_handle h, int radius)
         CU_TRY(cudaFuncSetAttribute(k0_equalise<uint8_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(OF_MAX_WINDOW_RADIUS, 1)));
         CU_TRY(cudaFuncSetAttribute(k0_equalise<uint16_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(OF_MAX_WINDOW_RADIUS, 2)));
         CU_TRY(cudaFuncSetAttribute(k0_equalise<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(OF_MAX_WINDOW_RADIUS, 4)));
+        CU_TRY(cudaFuncSetAttribute(k0_equalise<uint8_t, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(5, 1)));
+        CU_TRY(cudaFuncSetAttribute(k0_equalise<uint16_t, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)eq_smem_bytes(5, 2)));
     }
     h->eq_radius = radius;
     drop_graphs(h);

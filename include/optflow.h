@@ -107,6 +107,16 @@ int of_set_graph(of_handle h, int enable);
  * launch.  Both give bit-identical results. */
 int of_set_persistent(of_handle h, int enable);
 
+/* Hoist what does not change within a pyramid level out of its iterations (default off).  Ix, Iy are
+ * differences of I1 alone (reading D9 of DESIGN.md), so the planes IxIx, IxIy, IyIy -- and their
+ * window sums, the 2x2 matrix of the paper's local least-squares problem, PAPER.md:59-63 -- are the
+ * same in every iteration of a level; only IxIt, IyIt follow the warped I2.  With 1, the per-iteration
+ * product kernel forms and writes all five planes in the first iteration of a level and the two
+ * It planes afterwards (60 instead of 72 B per pixel-iteration; SURVEY.md 8(f) note f5).  The
+ * arithmetic of every value is unchanged: results are bit-identical to the default.  Off by default
+ * because BASELINE.json's north_star states the five-plane form per iteration. */
+int of_set_hoist(of_handle h, int enable);
+
 /* Validity bytes (1 = tr(G) > 0, D14) of the last iteration at level 0 of the last solve: copies
  * H x W bytes into the device buffer mask_dev, on `stream`. */
 int of_get_validity(of_handle h, uint8_t *mask_dev, void *stream);

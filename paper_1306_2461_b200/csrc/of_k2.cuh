@@ -45,6 +45,8 @@ struct K2Params {
     int dbg;                                       // profiling switches (0 in production): 1 = no product phase, 2 = no sum phase, 32 = no plane stores
     const uint8_t *mask;                           // obstacle mask of the level (pitch = `pitch`) or NULL (M2: zero weight)
     const int *list;                               // compacted tile list (then ntiles = its length) or NULL
+    int f_first;                                   // first plane this pass forms: 0 = all five; 3 = IxIt, IyIt only (of_set_hoist:
+                                                   // IxIx, IxIy, IyIy depend on I1 alone and keep their values of the level's first pass)
 };
 
 // Inputs of one phase-1 task (2 columns x 2 rows): I1 rows y-1..y+2 at columns x, x+1, the left and
@@ -223,7 +225,8 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
             }
             char *d = sm + rp * BB + cp * 16 + (cp >> 2) * 16;
 #pragma unroll
-            for (int f = 0; f < 5; ++f) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
+            for (int f = 0; f < 5; ++f)
+                if (f >= p.f_first) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
         }
         __syncwarp();
 
@@ -232,7 +235,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
             const int gx = x0 + 8 * h_seg, gy = y0 + 2 * h_rp;
             const char *src = sm + h_rp * BB + h_seg * 80;
 #pragma unroll 1
-            for (int f = h_f0; f < 5; f += nf_par) {
+            for (int f = p.f_first + h_f0; f < 5; f += nf_par) {
                 float2 in[G::NIN];
 #pragma unroll
                 for (int k = 0; k < G::NIN / 2; ++k) {

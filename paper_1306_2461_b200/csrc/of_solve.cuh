@@ -50,6 +50,7 @@ struct SolveArgs {
     SolveParams sp;
     const MaskDesc *md;                      // device array [levels]: obstacle masks and work lists (read by the MK kernel only;
                                              // last, so that every other field keeps its place in the parameter bank)
+    int hoist;                               // of_set_hoist: planes IxIx, IxIy, IyIy formed in the first iteration of a level only
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
@@ -202,10 +203,11 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             k3_b = cd.ent_b; k3_e = cd.ent_e; k3_chunks = (uint32_t)cd.nchunks;
         }
         K2Params p2 = {L.pyr[a.s1], L.pyr[a.s2], L.u, L.v, a.S, a.plane, L.W, L.H, L.pitch,
-                       L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, 0, a.dbg, M.mask, M.k2_list};
+                       L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, 0, a.dbg, M.mask, M.k2_list, 0};
         for (int it = 0; it < a.iterations; ++it) {
             // ---- K2 pass: warp + gradients + products + horizontal sums -> five planes
             p2.zero_uv = (l == top && it == 0) ? 1 : 0;            // zero initial guess at the coarsest level
+            p2.f_first = (a.hoist && it > 0) ? 3 : 0;
             k2_phase<R, MK>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             prof_stamp(a, pi);

@@ -108,6 +108,7 @@ struct of_context {
     unsigned long long *d_prof;         // timeline buffer of the persistent kernel (of_solve_timeline)
     bool prof_on;
     bool persistent;                    // whole solve in one cooperative launch (default) vs one launch per kernel
+    bool hoist;                         // of_set_hoist: IxIx, IxIy, IyIy planes formed once per level (default off)
     bool use_graph;
     std::vector<GraphEntry> graphs;
     unsigned long long stamp;
@@ -200,13 +201,13 @@ template <int R> void plan_level(of_context *c, int l)
 }
 
 template <int R>
-void launch_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
+void launch_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, int f_first, cudaStream_t st)
 {
     const Level &L = c->lv[l];
     const K2Plan &P = c->k2[l];
     const MaskDesc &M = c->md[l];
     K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, M.k2_list ? M.k2_n : P.ntiles,
-                  c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list};
+                  c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list, f_first};
     if (M.mask) k2_products_hsum<R, true><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
     else k2_products_hsum<R, false><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
 }
@@ -230,7 +231,7 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
     a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
     a.valid = c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
-    a.md = c->d_md;
+    a.md = c->d_md; a.hoist = c->hoist ? 1 : 0;
     a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
     a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
     void *args[] = {&a};
@@ -276,9 +277,9 @@ int encode_tensor_maps(of_context *c)
     default: break;                                                                                \
     }
 
-void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
+void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, int f_first, cudaStream_t st)
 {
-    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, zero_uv, st));
+    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, zero_uv, f_first, st));
 }
 void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st)
 {
@@ -392,7 +393,7 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
         if (l < top) { run_upsample(c, l, st); note_launch(c, "upsample", l); ++n; }
         for (int it = 0; it < c->iterations; ++it) {
             const bool zero_uv = (l == top && it == 0);
-            run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], zero_uv, st);
+            run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], zero_uv, (c->hoist && it > 0) ? 3 : 0, st);
             note_launch(c, "products+hsum", l);
             const bool last = (l == 0 && it == c->iterations - 1);
             if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, zero_uv, st);
@@ -831,6 +832,14 @@ int of_set_persistent(of_handle h, int enable)
     return OF_OK;
 }
 
+int of_set_hoist(of_handle h, int enable)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    h->hoist = enable != 0;
+    drop_graphs(h);
+    return OF_OK;
+}
+
 int of_solve_timeline(of_handle h, int enable, int cta, unsigned long long *out_host, int max_entries)
 {
     static_assert(OF_TIMELINE_MAX == SOLVE_TIMELINE_MAX, "timeline sizes out of sync");
@@ -894,7 +903,7 @@ int of_run_step(of_handle h, int level, int which, int repeat, void *stream)
     if (!h || level < 0 || level >= h->levels || which < 0 || which > 1 || repeat < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
     CU_TRY(cudaSetDevice(h->device));
     for (int i = 0; i < repeat; ++i) {
-        if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], false, (cudaStream_t)stream);
+        if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], false, 0, (cudaStream_t)stream);
         else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, false, (cudaStream_t)stream);
     }
     CU_TRY(cudaGetLastError());

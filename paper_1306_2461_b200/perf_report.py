@@ -1,6 +1,6 @@
 """Per-config throughput and in-kernel pass timeline of the solve (CUDA path only).
 
-    python -m paper_1306_2461_b200.perf_report [--configs 1 2 3 4] [--reps 50] [--masks]
+    python -m paper_1306_2461_b200.perf_report [--configs 1 2 3 4] [--reps 50] [--masks] [--hoist]
 
 For every config of BASELINE.json: frame pairs/s with device-resident inputs (CUDA events over `reps`
 solves), the persistent solve kernel alone (of_run_solve), its algorithmic GB/s on the 72 B per
@@ -17,7 +17,7 @@ import json
 import numpy as np
 
 
-def report(index: int, reps: int, sm_mhz: float, mask=None, mask_name=None):
+def report(index: int, reps: int, sm_mhz: float, mask=None, mask_name=None, hoist=False):
     import torch
     from . import binding as B, synthetic as syn
     c = syn.make_case(index)
@@ -32,6 +32,8 @@ def report(index: int, reps: int, sm_mhz: float, mask=None, mask_name=None):
     with B.OpticalFlow(*c.create_args) as of:
         if mask is not None:
             of.set_mask(mask)
+        of.set_hoist(hoist)
+        out["hoist"] = bool(hoist)
         s = torch.cuda.Stream()
         with torch.cuda.stream(s):
             u, v = of.compute(d1, d2)
@@ -82,6 +84,8 @@ def main():
     ap.add_argument("--configs", type=int, nargs="*", default=[1, 2, 3, 4])
     ap.add_argument("--reps", type=int, default=50)
     ap.add_argument("--sm-mhz", type=float, default=1965.0, help="SM clock used to convert cycle stamps")
+    ap.add_argument("--hoist", action="store_true", help="of_set_hoist(1): IxIx, IxIy, IyIy planes formed once per level (60 B basis; "
+                                                          "the GB/s figures printed here stay on the 72 B basis)")
     ap.add_argument("--masks", action="store_true", help="config 3 without a mask, with the step mask, with the right half masked")
     args = ap.parse_args()
     if args.masks:
@@ -89,10 +93,10 @@ def main():
         half = np.ones((1024, 1280), dtype=np.uint8)
         half[:, 640:] = 0
         for name, m in (("none", None), ("backward_step", syn.mask_backward_step(1280, 1024)), ("right_half", half)):
-            print(json.dumps(report(3, args.reps, args.sm_mhz, m, name)))
+            print(json.dumps(report(3, args.reps, args.sm_mhz, m, name, args.hoist)))
         return
     for k in args.configs:
-        print(json.dumps(report(k, args.reps, args.sm_mhz)))
+        print(json.dumps(report(k, args.reps, args.sm_mhz, hoist=args.hoist)))
 
 
 if __name__ == "__main__":

@@ -324,6 +324,33 @@ def test_persistent_and_per_kernel_launches_agree_bitwise(torch, B, W, H, L, R, 
     assert out[0][3] == prep + 1 and out[1][3] == prep + (L - 1) + 2 * L * it
 
 
+@pytest.mark.parametrize("W,H,L,R,it,wt,persistent", [(320, 256, 3, 12, 4, GAUSS, True), (130, 70, 2, 4, 3, BOX, True),
+                                                     (203, 131, 3, 8, 5, BOX, False), (1280, 1024, 3, 12, 10, GAUSS, True)])
+def test_hoisted_invariant_planes_agree_bitwise(torch, B, W, H, L, R, it, wt, persistent):
+    """of_set_hoist (SURVEY.md 8(f) note f5, reading D9): IxIx, IxIy, IyIy depend on I1 alone, so forming them in the
+    first iteration of a level only must not change a single bit of the result, with and without an obstacle mask."""
+    c = syn.config3(W, H)
+    d1, d2 = torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()
+    mask = np.ones((H, W), np.uint8)
+    mask[H // 3: H // 2, : W // 2] = 0
+    for use_mask in (False, True):
+        out = []
+        for hoist in (False, True):
+            with B.OpticalFlow(W, H, L, R, it, wt) as of:
+                of.set_persistent(persistent)
+                of.set_hoist(hoist)
+                if use_mask:
+                    of.set_mask(mask)
+                s = torch.cuda.Stream()
+                with torch.cuda.stream(s):
+                    for _ in range(2):                  # second solve: the planes of the previous pair must not leak in
+                        u, v = of.compute(d2 if _ == 0 else d1, d1 if _ == 0 else d2)
+                    m = of.validity()
+                s.synchronize()
+                out.append((u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy()))
+        assert all(np.array_equal(a, b) for a, b in zip(out[0], out[1])), "hoist changed the result (mask=%s)" % use_mask
+
+
 def test_large_image_crop_parity(torch, B, oracle):
     """4096x3072, one level: the result in a window depends only on a neighbourhood of radius
     iterations*(R+max|u|+2), so the oracle on a crop pins sampled outputs of the full-size run."""

@@ -46,7 +46,8 @@ struct K2Params {
     const uint8_t *mask;                           // obstacle mask of the level (pitch = `pitch`) or NULL (M2: zero weight)
     const int *list;                               // compacted tile list (then ntiles = its length) or NULL
     int f_first;                                   // first plane this pass forms: 0 = all five; 3 = IxIt, IyIt only (of_set_hoist:
-                                                   // IxIx, IxIy, IyIy depend on I1 alone and keep their values of the level's first pass)
+                                                   // IxIx, IxIy, IyIy depend on I1 alone and keep their values of the level's first
+                                                   // pass); read by the HO instantiation only
 };
 
 // Inputs of one phase-1 task (2 columns x 2 rows): I1 rows y-1..y+2 at columns x, x+1, the left and
@@ -181,11 +182,13 @@ template <bool MK> __device__ __forceinline__ void k2_task_products(const K2Para
 // kernel below and by the persistent solve kernel (of_solve.cuh).
 // MK = an obstacle mask is set (p.mask and p.list are valid): a separate instantiation, so that the unmasked
 // path carries none of the mask's instructions or registers.
-template <int R, bool MK>
+// HO = of_set_hoist: p.f_first selects the planes formed (0 otherwise, at compile time).
+template <int R, bool MK, bool HO>
 __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_cta, int *tile_counter, int warp, int lane, int t_begin, int t_end)
 {
     typedef K2Geom<R> G;
     const int nseg = p.nseg, nrp = p.nrp;
+    const int f_first = HO ? p.f_first : 0;
     const int PW = G::pw(nseg), half = PW >> 1, BB = G::block_bytes(nseg);
     char *const sm = reinterpret_cast<char *>(smem_cta) + warp * G::warp_bytes(nseg, nrp);
     const int W = p.W, H = p.H, pitch = p.pitch;
@@ -226,7 +229,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
             char *d = sm + rp * BB + cp * 16 + (cp >> 2) * 16;
 #pragma unroll
             for (int f = 0; f < 5; ++f)
-                if (f >= p.f_first) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
+                if (f >= f_first) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
         }
         __syncwarp();
 
@@ -235,7 +238,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
             const int gx = x0 + 8 * h_seg, gy = y0 + 2 * h_rp;
             const char *src = sm + h_rp * BB + h_seg * 80;
 #pragma unroll 1
-            for (int f = p.f_first + h_f0; f < 5; f += nf_par) {
+            for (int f = f_first + h_f0; f < 5; f += nf_par) {
                 float2 in[G::NIN];
 #pragma unroll
                 for (int k = 0; k < G::NIN / 2; ++k) {
@@ -286,5 +289,5 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
     __syncthreads();
     int t_begin, t_end;
     cta_range(p.ntiles, blockIdx.x, gridDim.x, t_begin, t_end);
-    k2_phase<R, MK>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, t_begin, t_end);
+    k2_phase<R, MK, false>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, t_begin, t_end);
 }

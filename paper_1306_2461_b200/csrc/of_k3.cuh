@@ -55,6 +55,8 @@ struct K3Params {
     int zero_uv;                     // 1 = the incoming field is identically zero and is not read (see of_k2.cuh)
     int dbg;                         // profiling switches (0 in production): 1 = no TMA/no waits, 2 = no window sum, 4 = no solve
     MaskDesc md;                     // obstacle mask and compacted task lists of the level (all zero: none)
+    float *G;                        // of_set_hoist: three planes (stride `gplane`, pitch `pitch`) holding the window sums a, b, c
+    size_t gplane;                   //   of IxIx, IxIy, IyIy of the level (written by an HM = 1 pass, read by HM = 2 passes)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -151,12 +153,18 @@ template <int R> __device__ __forceinline__ int k3_cta_chunks(int t_begin, int t
 // kernel (keeps slot / parity bookkeeping continuous); *sm.counter must be 0 on entry (CTA-synchronised).
 // All reads of u, v go through L2 (ld.global.cg): see of_k2.cuh.
 // MK = an obstacle mask is set (p.md is valid): a separate instantiation (cf. of_k2.cuh).
-template <int R, bool MK>
+// HM = hoisting mode (of_set_hoist; a, b, c are the same in every iteration of a level, reading D9):
+//   0: five planes in, nothing kept (default);  1: five planes in, a, b, c also stored to p.G (first iteration of a level);
+//   2: tmS is the two-plane map (box 64 x K3_SEG x 2) read at field 3: only IxIt, IyIt are fetched and summed, a, b, c come from p.G.
+// The value of every sum is formed by the same instructions in the same order in all three modes.
+template <int R, bool MK, int HM>
 __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params &p, const K3Smem &sm, int warp, int lane, int nwc,
                                          int t_begin, int t_end, uint32_t gc0)
 {
     typedef K3Geom<R> G;
     constexpr int NC = G::NC;
+    constexpr int F0 = HM == 2 ? 3 : 0;                  // first field fetched and summed
+    constexpr uint32_t CHUNK_TX = 64 * K3_SEG * (5 - F0) * 4;
     unsigned char *const k3_smem = sm.base;
     const uint32_t ring0 = sm.ring0, full0 = sm.full0, empty0 = sm.empty0;
     int *const counter = sm.counter;
@@ -177,8 +185,8 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
                     if (use > 0) mbar_wait(empty0 + 8 * slot, (use - 1) & 1);
                     const int readers = min(ntask - 1, c) - max(0, c - NC + 1) + 1;
                     if (readers < NC) mbar_arrive(empty0 + 8 * slot, NC - readers);   // stand-ins for tasks that do not exist
-                    mbar_expect_tx(full0 + 8 * slot, K3_CHUNK_BYTES);
-                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + K3_SEG * c, 0, full0 + 8 * slot);
+                    mbar_expect_tx(full0 + 8 * slot, CHUNK_TX);
+                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + K3_SEG * c, F0, full0 + 8 * slot);
                 }
             };
             if (MK) {                                                   // compacted lists: the host has cut the runs
@@ -230,6 +238,17 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             uu[j] = (active && !p.zero_uv) ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
             vv[j] = (active && !p.zero_uv) ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
         }
+        float2 ga[K3_SEG], gb[K3_SEG], gcc[K3_SEG];      // HM = 2: the level's a, b, c (L2 reads: written by another pass of this launch)
+        if (HM == 2) {
+            const float *gp = p.G + (size_t)gy0 * pitch + gx;
+#pragma unroll
+            for (int j = 0; j < K3_SEG; ++j) {
+                const int jj = min(j, nrows - 1) * pitch;
+                ga[j] = active ? __ldcg(reinterpret_cast<const float2 *>(gp + jj)) : make_float2(0.f, 0.f);
+                gb[j] = active ? __ldcg(reinterpret_cast<const float2 *>(gp + p.gplane + jj)) : make_float2(0.f, 0.f);
+                gcc[j] = active ? __ldcg(reinterpret_cast<const float2 *>(gp + 2 * p.gplane + jj)) : make_float2(0.f, 0.f);
+            }
+        }
         const unsigned char *cb[NC];
         uint32_t eb[NC], fb[NC], fpar[NC];
 #pragma unroll
@@ -250,8 +269,8 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         for (int r = 0; r < G::NIN; ++r) {
             if ((r % K3_SEG) == 0 && !(p.dbg & 1)) mbar_wait(fb[r / K3_SEG], fpar[r / K3_SEG]);   // chunk by chunk, as the TMA delivers them
 #pragma unroll
-            for (int f = 0; f < 5; ++f) {
-                const float2 val = *reinterpret_cast<const float2 *>(cb[r / K3_SEG] + f * (K3_SEG * 256) + (r % K3_SEG) * 256);
+            for (int f = F0; f < 5; ++f) {
+                const float2 val = *reinterpret_cast<const float2 *>(cb[r / K3_SEG] + (f - F0) * (K3_SEG * 256) + (r % K3_SEG) * 256);
 #pragma unroll
                 for (int j = 0; j < K3_SEG; ++j)
                     if (r - j >= 0 && r - j <= 2 * R) acc[f][j] = fma2s(p.ww.w[r - j], val, acc[f][j]);
@@ -263,6 +282,20 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             for (int k = 0; k < NC; ++k) mbar_arrive(eb[k], 1);
         }
         if (!active || (p.dbg & 4)) continue;
+        if (HM == 1) {                                   // keep a, b, c for the later iterations of the level
+            float *gp = p.G + (size_t)gy0 * pitch + gx;
+#pragma unroll
+            for (int j = 0; j < K3_SEG; ++j)
+                if (j < nrows) {
+                    *reinterpret_cast<float2 *>(gp + j * pitch) = acc[0][j];
+                    *reinterpret_cast<float2 *>(gp + p.gplane + j * pitch) = acc[1][j];
+                    *reinterpret_cast<float2 *>(gp + 2 * p.gplane + j * pitch) = acc[2][j];
+                }
+        }
+        if (HM == 2) {
+#pragma unroll
+            for (int j = 0; j < K3_SEG; ++j) { acc[0][j] = ga[j]; acc[1][j] = gb[j]; acc[2][j] = gcc[j]; }
+        }
         // ---- solve + update for K3_SEG rows x 2 columns
         const bool pair_ok = gx + 1 < W;
         const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
@@ -312,5 +345,5 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
     int t_begin, t_end;
     cta_range(p.ntasks, blockIdx.x, gridDim.x, t_begin, t_end);
     if (MK) { t_begin = p.md.k3_cta[blockIdx.x].ent_b; t_end = p.md.k3_cta[blockIdx.x].ent_e; }
-    k3_phase<R, MK>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, t_begin, t_end, 0u);
+    k3_phase<R, MK, 0>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, t_begin, t_end, 0u);
 }

@@ -50,7 +50,10 @@ struct SolveArgs {
     SolveParams sp;
     const MaskDesc *md;                      // device array [levels]: obstacle masks and work lists (read by the MK kernel only;
                                              // last, so that every other field keeps its place in the parameter bank)
-    int hoist;                               // of_set_hoist: planes IxIx, IxIy, IyIy formed in the first iteration of a level only
+    // of_set_hoist (HO instantiation only): the planes IxIt, IyIt of a level as an (x, y, field) tensor with a two-field
+    // box, and the three planes that keep the level's window sums a, b, c
+    float *G;
+    alignas(64) CUtensorMap tm2[SOLVE_MAX_LEVELS];
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
@@ -166,7 +169,10 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
 }
 
 // MK = an obstacle mask is set (of_set_mask): compacted work lists, masked products / outputs.
-template <int R, bool MK>
+// HO = of_set_hoist: IxIx, IxIy, IyIy and their window sums a, b, c are formed in the first iteration of a level only
+// (they depend on I1 alone, reading D9): later iterations write, fetch and sum the two It planes (60 B per pixel-iteration
+// instead of 72).  A separate instantiation: the default kernel carries none of it.
+template <int R, bool MK, bool HO>
 __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __grid_constant__ SolveArgs a)
 {
     extern __shared__ __align__(1024) unsigned char solve_smem[];
@@ -207,8 +213,8 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
         for (int it = 0; it < a.iterations; ++it) {
             // ---- K2 pass: warp + gradients + products + horizontal sums -> five planes
             p2.zero_uv = (l == top && it == 0) ? 1 : 0;            // zero initial guess at the coarsest level
-            p2.f_first = (a.hoist && it > 0) ? 3 : 0;
-            k2_phase<R, MK>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
+            p2.f_first = (HO && it > 0) ? 3 : 0;
+            k2_phase<R, MK, HO>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             prof_stamp(a, pi);
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
@@ -216,9 +222,11 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             // ---- K3 pass: vertical sums + solve + update
             const bool last = (l == 0 && it == a.iterations - 1);
             K3Params p3 = {L.u, L.v, last ? a.u_out : L.u, last ? a.v_out : L.v, last ? a.valid : nullptr, last ? a.det : nullptr,
-                           L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, p2.zero_uv, a.dbg, M};
+                           L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, p2.zero_uv, a.dbg, M, HO ? a.G : nullptr, a.plane};
             if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async.global;" ::: "memory");
-            k3_phase<R, MK>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            if (!HO) k3_phase<R, MK, 0>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            else if (it == 0) k3_phase<R, MK, 1>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            else k3_phase<R, MK, 2>(&a.tm2[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
             gc0 += k3_chunks;
             __syncthreads();
             if (threadIdx.x == 0) { sm.counter[0] = 0; sm.counter[1] = 0; }

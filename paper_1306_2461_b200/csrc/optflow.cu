@@ -108,7 +108,9 @@ struct of_context {
     unsigned long long *d_prof;         // timeline buffer of the persistent kernel (of_solve_timeline)
     bool prof_on;
     bool persistent;                    // whole solve in one cooperative launch (default) vs one launch per kernel
-    bool hoist;                         // of_set_hoist: IxIx, IxIy, IyIy planes formed once per level (default off)
+    bool hoist;                         // of_set_hoist: IxIx, IxIy, IyIy planes and their sums formed once per level (default off)
+    float *G;                           // three planes for the level's window sums a, b, c (allocated by of_set_hoist)
+    CUtensorMap tmS2[OF_MAX_LEVELS];    // planes 3, 4 (IxIt, IyIt) of a level as an (x, y, field) tensor with a two-field box
     bool use_graph;
     std::vector<GraphEntry> graphs;
     unsigned long long stamp;
@@ -130,10 +132,12 @@ template <int R> int setup_attrs()
 {
     CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
 }
 
@@ -201,13 +205,13 @@ template <int R> void plan_level(of_context *c, int l)
 }
 
 template <int R>
-void launch_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, int f_first, cudaStream_t st)
+void launch_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
 {
     const Level &L = c->lv[l];
     const K2Plan &P = c->k2[l];
     const MaskDesc &M = c->md[l];
     K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, M.k2_list ? M.k2_n : P.ntiles,
-                  c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list, f_first};
+                  c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list, 0};
     if (M.mask) k2_products_hsum<R, true><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
     else k2_products_hsum<R, false><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
 }
@@ -218,7 +222,7 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     const Level &L = c->lv[l];
     const K3Plan &P = c->k3[l];
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
-                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg, c->md[l]};
+                  L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg, c->md[l], nullptr, 0};
     if (c->md[l].mask) k3_vsum_solve<R, true><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
     else k3_vsum_solve<R, false><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
@@ -231,11 +235,15 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
     a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
     a.valid = c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
-    a.md = c->d_md; a.hoist = c->hoist ? 1 : 0;
+    a.md = c->d_md; a.G = c->G;
+    const bool ho = c->hoist && c->G != nullptr;
+    if (ho) memcpy(a.tm2, c->tmS2, sizeof(CUtensorMap) * c->levels);
     a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
     a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
     void *args[] = {&a};
-    return cudaLaunchCooperativeKernel(c->md[0].mask ? (const void *)of_solve_pair<R, true> : (const void *)of_solve_pair<R, false>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
+    const void *fn = c->md[0].mask ? (ho ? (const void *)of_solve_pair<R, true, true> : (const void *)of_solve_pair<R, true, false>)
+                                   : (ho ? (const void *)of_solve_pair<R, false, true> : (const void *)of_solve_pair<R, false, false>);
+    return cudaLaunchCooperativeKernel(fn, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
                                        (size_t)K3Geom<R>::SMEM, st);
 }
 
@@ -260,6 +268,11 @@ int encode_tensor_maps(of_context *c)
                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(OF_ERR_CUDA, "cuTensorMapEncodeTiled(level %d) failed: CUresult %d", l, (int)r);
+        cuuint32_t box2[3] = {64, K3_SEG, 2};                   // of_set_hoist: the two It planes fetched at field 3
+        r = ((encode_fn)fn)(&c->tmS2[l], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, c->S, dims, strides, box2, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(OF_ERR_CUDA, "cuTensorMapEncodeTiled(level %d, two-field box) failed: CUresult %d", l, (int)r);
     }
     return OF_OK;
 }
@@ -277,9 +290,9 @@ int encode_tensor_maps(of_context *c)
     default: break;                                                                                \
     }
 
-void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, int f_first, cudaStream_t st)
+void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
 {
-    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, zero_uv, f_first, st));
+    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, zero_uv, st));
 }
 void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st)
 {
@@ -393,7 +406,7 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
         if (l < top) { run_upsample(c, l, st); note_launch(c, "upsample", l); ++n; }
         for (int it = 0; it < c->iterations; ++it) {
             const bool zero_uv = (l == top && it == 0);
-            run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], zero_uv, (c->hoist && it > 0) ? 3 : 0, st);
+            run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], zero_uv, st);
             note_launch(c, "products+hsum", l);
             const bool last = (l == 0 && it == c->iterations - 1);
             if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, zero_uv, st);
@@ -835,6 +848,11 @@ int of_set_persistent(of_handle h, int enable)
 int of_set_hoist(of_handle h, int enable)
 {
     if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    if (enable && !h->G) {
+        CU_TRY(cudaSetDevice(h->device));
+        int rc = dev_alloc(h, (void **)&h->G, sizeof(float) * 3 * h->plane);
+        if (rc != OF_OK) return rc;
+    }
     h->hoist = enable != 0;
     drop_graphs(h);
     return OF_OK;
@@ -903,7 +921,7 @@ int of_run_step(of_handle h, int level, int which, int repeat, void *stream)
     if (!h || level < 0 || level >= h->levels || which < 0 || which > 1 || repeat < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
     CU_TRY(cudaSetDevice(h->device));
     for (int i = 0; i < repeat; ++i) {
-        if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], false, 0, (cudaStream_t)stream);
+        if (which == 0) run_k2(h, level, h->pyr[0][level], h->pyr[1][level], false, (cudaStream_t)stream);
         else run_k3(h, level, h->u[level], h->v[level], h->lv[level].pitch, false, false, (cudaStream_t)stream);
     }
     CU_TRY(cudaGetLastError());

@@ -229,6 +229,36 @@ def run_ours(args):
         of.compute(d_in[0][0], d_in[0][1], d_out[0][0], d_out[0][1])
     stream.synchronize()
     tl = of.solve_timeline(False).astype(np.float64)
+
+    # ---------------- the same job with of_set_hoist(1) (opt-in; bit-identical results; reported beside the headline, which
+    # stays the five-plane form BASELINE.json's north_star states)
+    hoist = None
+    if not args.no_hoist:
+        of.set_hoist(True)
+        with torch.cuda.stream(stream):
+            for i in range(3 + RING):
+                of.compute(d_in[i % RING][0], d_in[i % RING][1], d_out[i % RING][0], d_out[i % RING][1])
+            h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            h0.record()
+            for i in range(args.steps):
+                of.compute(d_in[i % RING][0], d_in[i % RING][1], d_out[i % RING][0], d_out[i % RING][1])
+            h1.record()
+            h1.synchronize()
+            h_ms = h0.elapsed_time(h1)
+            of.run_solve(5)
+            h0.record()
+            of.run_solve(100)
+            h1.record()
+            h1.synchronize()
+            h_solve_us = h0.elapsed_time(h1) / 100 * 1e3
+        of.solve_timeline(True)
+        with torch.cuda.stream(stream):
+            of.compute(d_in[0][0], d_in[0][1], d_out[0][0], d_out[0][1])
+        stream.synchronize()
+        h_tl = of.solve_timeline(False).astype(np.float64)
+        of.set_hoist(False)
+        h_ms = reduce_max_time(h_ms, dist, dev)
+        hoist = (h_ms, h_solve_us, h_tl)
     clocks = sampler.stop()
     ms = reduce_max_time(ms, dist, dev)
 
@@ -296,6 +326,27 @@ def run_ours(args):
         iter_gbs = 72.0 * px / (iter_us * 1e-6) / 1e9
         pix_iters = sum(((W + (1 << l) - 1) >> l) * ((H + (1 << l) - 1) >> l) for l in range(c0.levels)) * c0.iterations
         value = world * args.steps / (ms * 1e-3)
+        hoist_out = None
+        if hoist is not None:
+            h_ms, h_solve_us, h_tl = hoist
+            hd = np.diff(h_tl) / mhz
+            hseg = hd[i0:i0 + 4 * it].reshape(it, 4)
+            hmed = np.median(hseg[1:-1], axis=0)               # iterations 2 .. it-1 of level 0 (the first one forms all five planes)
+            h_iter_us = float(hmed.sum())
+            # bytes moved with hoisting: first iteration of a level 72 + 12 (a, b, c written), later ones K2 16 R + 8 W, K3 28 R + 8 W
+            h_bytes = (84.0 + 60.0 * (it - 1)) * sum(level_px)
+            hoist_out = {"api": "of_set_hoist(handle, 1): IxIx, IxIy, IyIy and their window sums formed in the first iteration of a "
+                                "level only (SURVEY.md 8(f) note f5); results bit-identical to the headline run "
+                                "(tests/test_gpu_parity.py::test_hoisted_invariant_planes_agree_bitwise); opt-in",
+                         "value": world * args.steps / (h_ms * 1e-3), "unit": UNIT, "ms_per_step": h_ms / args.steps,
+                         "kernel": "of_solve_pair<12, false, true>", "us_per_launch": h_solve_us,
+                         "bytes_per_launch": h_bytes, "achieved_GB/s": h_bytes / (h_solve_us * 1e-6) / 1e9,
+                         "frac": h_bytes / (h_solve_us * 1e-6) / 1e9 / peak,
+                         "iteration_level0": {"us": h_iter_us, "bytes": 60 * px, "GB/s": 60.0 * px / (h_iter_us * 1e-6) / 1e9,
+                                              "frac_of_peak": 60.0 * px / (h_iter_us * 1e-6) / 1e9 / peak,
+                                              "frac_of_peak_on_72B_basis": 72.0 * px / (h_iter_us * 1e-6) / 1e9 / peak,
+                                              "phases_us": {"k2_pass": float(hmed[0]), "barrier_1": float(hmed[1]),
+                                                            "k3_pass": float(hmed[2]), "barrier_2": float(hmed[3])}}}
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -310,7 +361,7 @@ def run_ours(args):
                     "d2h_bytes_per_step": 8 * px, "steps": e2e_steps,
                     "api": "of_stream_open(PAIRS, host results) / acquire+fill / submit / result", "checksum": checksum},
             "gpu_launches": launches,
-            "roofline": {"bound": "hbm", "kernel": "of_solve_pair<12, false> (persistent: K2 pass + K3 pass + hand-down, all levels and iterations)",
+            "roofline": {"bound": "hbm", "kernel": "of_solve_pair<12, false, false> (persistent: K2 pass + K3 pass + hand-down, all levels and iterations)",
                          "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                          "traffic": NCU_DRAM_BYTES_PER_SOLVE, "traffic_source": "profiles/r1_persistent_solve.md (ncu --set full, dram read + write of one launch; the 47 MB of planes are L2 resident)",
                          "peak_source": peak_src, "bytes_per_launch": solve_bytes,
@@ -320,6 +371,7 @@ def run_ours(args):
                                  "phases_us": {"k2_pass": float(med[0]), "barrier_1": float(med[1]), "k3_pass": float(med[2]), "barrier_2": float(med[3])},
                                  "how": "in-kernel SM cycle stamps (of_solve_timeline, max over CTAs) / sampled SM clock; median over iterations"},
             "kernels_level0_standalone_us": kt,
+            "variant_hoist": hoist_out,
             "cpu_baseline": cpu,
         }
         print(json.dumps(out))
@@ -337,6 +389,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer pipeline leg (profiling runs)")
+    ap.add_argument("--no-hoist", action="store_true", help="skip the of_set_hoist(1) variant leg (profiling runs)")
     ap.add_argument("--ring", type=int, default=RING, help="distinct input pairs / output buffers cycled through")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -325,7 +325,8 @@ def test_persistent_and_per_kernel_launches_agree_bitwise(torch, B, W, H, L, R, 
 
 
 @pytest.mark.parametrize("W,H,L,R,it,wt,persistent", [(320, 256, 3, 12, 4, GAUSS, True), (130, 70, 2, 4, 3, BOX, True),
-                                                     (203, 131, 3, 8, 5, BOX, False), (1280, 1024, 3, 12, 10, GAUSS, True)])
+                                                     (203, 131, 3, 8, 5, BOX, False), (256, 256, 4, 10, 3, BOX, True),
+                                                     (1280, 1024, 3, 12, 10, GAUSS, True)])
 def test_hoisted_invariant_planes_agree_bitwise(torch, B, W, H, L, R, it, wt, persistent):
     """of_set_hoist (SURVEY.md 8(f) note f5, reading D9): IxIx, IxIy, IyIy depend on I1 alone, so forming them in the
     first iteration of a level only must not change a single bit of the result, with and without an obstacle mask."""

@@ -10,6 +10,9 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liboptflow.so")
 SOURCES = ["optflow.cu"]
 DEPS = ["optflow.cu", "of_kernels.cuh", "of_common.cuh", "of_k2.cuh", "of_k3.cuh", "of_solve.cuh", "of_equalise.cuh", "of_post.cuh", os.path.join("..", "..", "include", "optflow.h")]
+# OF_NVCC_DEFS="--split-compile 8" cuts the build from ~140 s to ~50 s, but nvcc then picks a different register allocation from
+# run to run (measured: 156/160, 162/156 or 166/168 registers for the two R = 12 solve kernels), so it is not the default:
+# the library that is tested must be the library that is rebuilt from the same sources.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 

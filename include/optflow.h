@@ -114,7 +114,10 @@ int of_set_persistent(of_handle h, int enable);
  * product kernel forms and writes all five planes in the first iteration of a level and the two
  * It planes afterwards (60 instead of 72 B per pixel-iteration; SURVEY.md 8(f) note f5).  The
  * arithmetic of every value is unchanged: results are bit-identical to the default.  Off by default
- * because BASELINE.json's north_star states the five-plane form per iteration. */
+ * because BASELINE.json's north_star states the five-plane form per iteration.  The first call with 1
+ * allocates three more planes (the level's window sums a, b, c) on the handle's device.  Applies to the
+ * persistent solve kernel; with of_set_persistent(h, 0) every pass forms all five planes.  Returns OF_OK
+ * or an error code (OF_ERR_CUDA if the allocation fails; the setting is then unchanged). */
 int of_set_hoist(of_handle h, int enable);
 
 /* Validity bytes (1 = tr(G) > 0, D14) of the last iteration at level 0 of the last solve: copies

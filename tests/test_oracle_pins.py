@@ -594,6 +594,34 @@ def test_masked_solve_equals_stepwise_composition(oracle):
     assert np.array_equal(u, r["u"]) and np.array_equal(v, r["v"]) and np.array_equal(valid, r["valid"])
 
 
+# ------------------------------------------------------------------ D9 (what of_set_hoist relies on)
+@pytest.mark.parametrize("wt,R", [(BOX, 4), (GAUSS, 6)])
+def test_matrix_sums_do_not_depend_on_the_displacement(oracle, wt, R):
+    """Reading D9: the gradients are taken on the unwarped I1, so the window sums a, b, c of IxIx, IxIy, IyIy (the 2x2
+    matrix of the local least-squares problem) are the same for every displacement field, i.e. in every
+    iteration of a level; only the sums of IxIt, IyIt follow the warp.  Pinned on the oracle itself: a, b, c with a zero
+    field equal a, b, c with a rough random field bit for bit (also with an obstacle mask), p and q do not, and a, b, c
+    equal the window sums of the gradient products formed here from np.gradient-style differences."""
+    c = syn.config1(72, 56)
+    I1, I2 = c.I1.astype(np.float64), c.I2.astype(np.float64)
+    rng = np.random.default_rng(7)
+    z = np.zeros_like(I1)
+    u, v = rng.uniform(-3, 3, I1.shape), rng.uniform(-3, 3, I1.shape)
+    mask = np.ones(I1.shape, np.uint8)
+    mask[20:30, 10:40] = 0
+    for m in (None, mask):
+        s0 = oracle.iteration(I1, I2, z, z, R, wt, mask=m)[2]
+        s1 = oracle.iteration(I1, I2, u, v, R, wt, mask=m)[2]
+        assert np.array_equal(s0[:3], s1[:3])
+        assert not np.array_equal(s0[3], s1[3]) and not np.array_equal(s0[4], s1[4])
+    # independent formation of a, b, c: central differences with clamped borders, then the oracle's own window sum
+    P = np.pad(I1, 1, mode="edge")
+    Ix, Iy = 0.5 * (P[1:-1, 2:] - P[1:-1, :-2]), 0.5 * (P[2:, 1:-1] - P[:-2, 1:-1])
+    s0 = oracle.iteration(I1, I2, u, v, R, wt)[2]
+    for k, f in enumerate((Ix * Ix, Ix * Iy, Iy * Iy)):
+        assert np.allclose(s0[k], oracle.window_sum(f, R, wt, direct=True), rtol=1e-12, atol=1e-9)
+
+
 def test_backward_step_mask_recipe():
     m = syn.mask_backward_step(1280, 1024)
     assert m.dtype == np.uint8 and m.shape == (1024, 1280)

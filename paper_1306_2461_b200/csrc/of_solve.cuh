@@ -90,10 +90,16 @@ __device__ __forceinline__ void grid_barrier_exit(unsigned *bar, unsigned ncta)
 
 __device__ __forceinline__ void prof_stamp(const SolveArgs &a, int &idx)
 {
-    if (a.prof != nullptr) __syncthreads();                      // stamp when the whole CTA is done, not just warp 0
-    if (a.prof != nullptr && threadIdx.x == 0) {
-        // SM cycle counter: %globaltimer is refreshed too coarsely (several us) to time a pass
-        a.prof[(size_t)blockIdx.x * SOLVE_TIMELINE_MAX + idx] = (unsigned long long)clock64();
+    if (a.prof != nullptr) {
+        // stamp when the whole CTA is done, not just warp 0: the clock read consumes the barrier's reduction result, so it cannot
+        // be issued before the barrier has released (a plain bar.sync lets the warp run ahead to the clock read)
+        const int n = __syncthreads_count(1);
+        if (threadIdx.x == 0) {
+            // SM cycle counter: %globaltimer is refreshed too coarsely (several us) to time a pass
+            unsigned long long t;
+            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %1, 0;\n\t@p mov.u64 %0, %%clock64;\n\t@!p mov.u64 %0, 0;\n\t}" : "=l"(t) : "r"(n) : "memory");
+            a.prof[(size_t)blockIdx.x * SOLVE_TIMELINE_MAX + idx] = t;
+        }
     }
     ++idx;
 }

@@ -34,7 +34,7 @@ METRIC = "dense-flow frame pairs/s at 1280x1024"
 UNIT = "pairs/s"
 WORKLOAD = "config3: 1280x1024 uint8 particle pair, backward-facing-step-like field, 3 levels, Gaussian window sigma 4 (R=12), 10 iterations"
 BYTES_PER_PX = {"k2_products_hsum": 16 + 20, "k3_vsum_solve": 28 + 8}    # 72 B per pixel-iteration
-NCU_DRAM_BYTES_PER_SOLVE = 13.83e6 + 11.37e6   # dram__bytes_read.sum + dram__bytes_write.sum, one of_solve_pair launch (profiles/)
+NCU_DRAM_BYTES_PER_SOLVE = 13.82e6 + 9.36e6   # dram__bytes_read.sum + dram__bytes_write.sum, one of_solve_pair launch (profiles/)
 RING = 16          # default: distinct input pairs + output buffers cycled through: 16*(2.6+10.5) MB = 210 MB > 126 MB L2
 
 
@@ -363,7 +363,7 @@ def run_ours(args):
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "kernel": "of_solve_pair<12, false, false> (persistent: K2 pass + K3 pass + hand-down, all levels and iterations)",
                          "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                         "traffic": NCU_DRAM_BYTES_PER_SOLVE, "traffic_source": "profiles/r1_persistent_solve.md (ncu --set full, dram read + write of one launch; the 47 MB of planes are L2 resident)",
+                         "traffic": NCU_DRAM_BYTES_PER_SOLVE, "traffic_source": "profiles/r1_persistent_solve.md, final-build addendum (ncu --set full, dram read + write of one launch; the 47 MB of planes are L2 resident)",
                          "peak_source": peak_src, "bytes_per_launch": solve_bytes,
                          "bytes_basis": "72 B per pixel-iteration (K2 16 R + 20 W, K3 28 R + 8 W) x %d pixel-iterations" % (sum(level_px) * c0.iterations),
                          "us_per_launch": solve_us},

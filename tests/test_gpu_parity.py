@@ -326,6 +326,7 @@ def test_persistent_and_per_kernel_launches_agree_bitwise(torch, B, W, H, L, R, 
 
 @pytest.mark.parametrize("W,H,L,R,it,wt,persistent", [(320, 256, 3, 12, 4, GAUSS, True), (130, 70, 2, 4, 3, BOX, True),
                                                      (203, 131, 3, 8, 5, BOX, False), (256, 256, 4, 10, 3, BOX, True),
+                                                     (37, 23, 1, 2, 1, BOX, True), (70, 67, 2, 16, 2, GAUSS, True),
                                                      (1280, 1024, 3, 12, 10, GAUSS, True)])
 def test_hoisted_invariant_planes_agree_bitwise(torch, B, W, H, L, R, it, wt, persistent):
     """of_set_hoist (SURVEY.md 8(f) note f5, reading D9): IxIx, IxIy, IyIy depend on I1 alone, so forming them in the

@@ -19,6 +19,9 @@
 #pragma once
 #include "of_common.cuh"
 
+#ifndef K2_AHEAD_MIN_ROUNDS
+#define K2_AHEAD_MIN_ROUNDS 2                      // tiles with more product rounds than this request u, v of all rounds up front
+#endif
 #ifndef K2_MAX_WARPS
 #define K2_MAX_WARPS 12                            // warps per CTA (independent of each other); runtime blockDim
 #endif
@@ -69,7 +72,7 @@ __device__ __forceinline__ const float *ptr_at(const float *base, int idx)
     return r;
 }
 
-template <bool MK> __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
+template <bool MK, bool LOADUV = true> __device__ __forceinline__ K2In k2_load(const K2Params &p, int x, int y)
 {
     K2In in;
     const int W = p.W, H = p.H, pitch = p.pitch;
@@ -80,7 +83,7 @@ template <bool MK> __device__ __forceinline__ K2In k2_load(const K2Params &p, in
     in.c0 = __ldg(reinterpret_cast<const float2 *>(c));
     in.c1 = __ldg(reinterpret_cast<const float2 *>(c1p));
     in.c2 = __ldg(reinterpret_cast<const float2 *>(ptr_at(c, d2)));
-    if (p.zero_uv) {
+    if (p.zero_uv || !LOADUV) {
         in.u0 = in.u1 = in.v0 = in.v1 = make_float2(0.f, 0.f);
     } else {
         const float *pu = ptr_at(p.u, i0), *pv = ptr_at(p.v, i0);
@@ -211,6 +214,53 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
         // ---------------- phase 1: products of (PW x TH) pixels -> shared memory
         // task k -> (row pair rp, column pair cp): input loads, then the 16 gathers of its four pixels,
         // then the arithmetic (other warps of the SM cover the two memory latencies)
+        if (ntasks > 32 * K2_AHEAD_MIN_ROUNDS) {
+        // wide tiles (three or more product rounds): the field values of ALL rounds of the tile are requested first, so that a
+        // round's gathers wait for one L2 round trip (I1 / I2) instead of two (u, v, then I2).  Measured (profiles/r1_experiments.md):
+        // level-0 K2 pass 16.0 -> 15.1 us at 1280x1024, 57.2 -> 50.1 us at 2048x2048; one-round tiles of the coarse levels lose
+        // 0.4 us with it (unrolled guards), so they keep the rolled loop below.
+        constexpr int MAXR = 6;
+        float2 pu0[MAXR], pu1[MAXR], pv0[MAXR], pv1[MAXR];
+#pragma unroll
+        for (int r = 0; r < MAXR; ++r) {
+            pu0[r] = pu1[r] = pv0[r] = pv1[r] = make_float2(0.f, 0.f);
+            const int k = lane + 32 * r;
+            int rp = 0, cp = k;
+            while (cp >= half) { cp -= half; ++rp; }
+            const int x = xs + 2 * cp, y = y0 + 2 * rp;
+            if (k < ntasks && !p.zero_uv && x >= 0 && x < W && y < H) {
+                const int i0 = y * pitch + x, d1 = y + 1 < H ? pitch : 0;
+                const float *qu = ptr_at(p.u, i0), *qv = ptr_at(p.v, i0);
+                pu0[r] = __ldcg(reinterpret_cast<const float2 *>(qu));
+                pu1[r] = __ldcg(reinterpret_cast<const float2 *>(ptr_at(qu, d1)));
+                pv0[r] = __ldcg(reinterpret_cast<const float2 *>(qv));
+                pv1[r] = __ldcg(reinterpret_cast<const float2 *>(ptr_at(qv, d1)));
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < MAXR; ++r) {
+            const int k = lane + 32 * r;
+            if (32 * r >= ntasks || k >= ntasks || (p.dbg & 1)) continue;
+            int rp = 0, cp = k;
+            while (cp >= half) { cp -= half; ++rp; }
+            const int x = xs + 2 * cp, y = y0 + 2 * rp;
+            float4 o[5];
+            if (x >= 0 && x < W && y < H) {
+                K2In in = k2_load<MK, false>(p, x, y);
+                in.u0 = pu0[r]; in.u1 = pu1[r]; in.v0 = pv0[r]; in.v1 = pv1[r];
+                K2Tap t[4];
+                k2_task_gather(p, in, x, y, t);
+                k2_task_products<MK>(p, in, x, y, t, o);
+            } else {
+#pragma unroll
+                for (int f = 0; f < 5; ++f) o[f] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            char *d = sm + rp * BB + cp * 16 + (cp >> 2) * 16;
+#pragma unroll
+            for (int f = 0; f < 5; ++f)
+                if (f >= f_first) *reinterpret_cast<float4 *>(d + f * nrp * BB) = o[f];
+        }
+        } else
 #pragma unroll 1
         for (int k = lane; k < ntasks && !(p.dbg & 1); k += 32) {
             int rp = 0, cp = k;

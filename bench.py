@@ -34,7 +34,7 @@ METRIC = "dense-flow frame pairs/s at 1280x1024"
 UNIT = "pairs/s"
 WORKLOAD = "config3: 1280x1024 uint8 particle pair, backward-facing-step-like field, 3 levels, Gaussian window sigma 4 (R=12), 10 iterations"
 BYTES_PER_PX = {"k2_products_hsum": 16 + 20, "k3_vsum_solve": 28 + 8}    # 72 B per pixel-iteration
-NCU_DRAM_BYTES_PER_SOLVE = 13.82e6 + 9.36e6   # dram__bytes_read.sum + dram__bytes_write.sum, one of_solve_pair launch (profiles/)
+NCU_DRAM_BYTES_PER_SOLVE = 13.85e6 + 11.26e6   # dram__bytes_read.sum + dram__bytes_write.sum, one of_solve_pair launch (profiles/)
 RING = 16          # default: distinct input pairs + output buffers cycled through: 16*(2.6+10.5) MB = 210 MB > 126 MB L2
 
 

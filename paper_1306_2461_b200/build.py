@@ -8,13 +8,13 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liboptflow.so")
-SOURCES = ["optflow.cu"]
-DEPS = ["optflow.cu", "of_kernels.cuh", "of_common.cuh", "of_k2.cuh", "of_k3.cuh", "of_solve.cuh", "of_equalise.cuh", "of_post.cuh", os.path.join("..", "..", "include", "optflow.h")]
+SOURCES = ["optflow.cu", "optflow_hoist.cu"]     # compiled in parallel (one nvcc process each), then linked
+DEPS = ["optflow.cu", "optflow_hoist.cu", "of_dispatch.cuh", "of_kernels.cuh", "of_common.cuh", "of_k2.cuh", "of_k3.cuh", "of_solve.cuh", "of_equalise.cuh", "of_post.cuh", os.path.join("..", "..", "include", "optflow.h")]
 # OF_NVCC_DEFS="--split-compile 8" cuts the build from ~140 s to ~50 s, but nvcc then picks a different register allocation from
 # run to run (measured: 156/160, 162/156 or 166/168 registers for the two R = 12 solve kernels), so it is not the default:
 # the library that is tested must be the library that is rebuilt from the same sources.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
 def _stale() -> bool:
@@ -28,13 +28,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("OF_NVCC_DEFS", "").split() + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
-        r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+        defs = os.environ.get("OF_NVCC_DEFS", "").split()
+        objs = [os.path.join(HERE, "build", os.path.splitext(src)[0] + ".o") for src in SOURCES]
+        os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+        cmds = [[nvcc] + NVCC_FLAGS + defs + ["-c", "-o", o, os.path.join(CSRC, src)] for src, o in zip(SOURCES, objs)]
+        procs = [subprocess.Popen(c, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for c in cmds]
+        outs = [pr.communicate()[0] for pr in procs]
+        rc = max(pr.returncode for pr in procs)
+        link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs
+        if rc == 0:
+            r = subprocess.run(link, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+            outs.append(r.stdout)
+            rc = r.returncode
+        log = "".join(" ".join(c) + "\n" + o for c, o in zip(cmds + [link], outs))
         with open(os.path.join(HERE, "build.log"), "w") as f:
-            f.write(" ".join(cmd) + "\n" + r.stdout)
-        if verbose or r.returncode != 0:
-            sys.stderr.write(r.stdout)
-        if r.returncode != 0:
+            f.write(log)
+        if verbose or rc != 0:
+            sys.stderr.write(log)
+        if rc != 0:
             raise RuntimeError("nvcc failed (see %s)" % os.path.join(HERE, "build.log"))
         os.replace(tmp, LIB)
     return LIB

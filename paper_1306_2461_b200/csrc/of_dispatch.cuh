@@ -1,0 +1,22 @@
+// of_dispatch.cuh -- radius dispatch (a run-time window radius selects a template instantiation) and the entry points of the
+// second translation unit.  The hoisted (of_set_hoist) instantiations of the persistent solve kernel are compiled in
+// optflow_hoist.cu, in parallel with optflow.cu: they are half of the build time and share nothing but headers with the rest.
+#pragma once
+#include "of_solve.cuh"
+
+#define DISPATCH_R(R_, CALL)                                                                       \
+    switch (R_) {                                                                                  \
+    case 1: { constexpr int R = 1; CALL; } break;   case 2: { constexpr int R = 2; CALL; } break;   \
+    case 3: { constexpr int R = 3; CALL; } break;   case 4: { constexpr int R = 4; CALL; } break;   \
+    case 5: { constexpr int R = 5; CALL; } break;   case 6: { constexpr int R = 6; CALL; } break;   \
+    case 7: { constexpr int R = 7; CALL; } break;   case 8: { constexpr int R = 8; CALL; } break;   \
+    case 9: { constexpr int R = 9; CALL; } break;   case 10: { constexpr int R = 10; CALL; } break; \
+    case 11: { constexpr int R = 11; CALL; } break; case 12: { constexpr int R = 12; CALL; } break; \
+    case 13: { constexpr int R = 13; CALL; } break; case 14: { constexpr int R = 14; CALL; } break; \
+    case 15: { constexpr int R = 15; CALL; } break; case 16: { constexpr int R = 16; CALL; } break; \
+    default: break;                                                                                \
+    }
+
+// optflow_hoist.cu: of_solve_pair<R, mk, true>.  Launch (cooperative, `sms` CTAs) and one-time attribute set-up.
+cudaError_t of_launch_solve_hoisted(int R, bool mk, const SolveArgs &a, int sms, cudaStream_t st);
+cudaError_t of_setup_attrs_hoisted(int R, int smem_max);

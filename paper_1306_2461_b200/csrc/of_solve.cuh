@@ -125,7 +125,7 @@ __device__ __forceinline__ void mask_zero_tasks(const int *zl, int n, int nrb, i
     }
 }
 
-__global__ void __launch_bounds__(256) k_mask_zero(const int *zl, int n, int nrb, int W, int H, int pitch, float *u_out, float *v_out,
+static __global__ void __launch_bounds__(256) k_mask_zero(const int *zl, int n, int nrb, int W, int H, int pitch, float *u_out, float *v_out,
                                                    int out_pitch, uint8_t *valid, float *det)
 {
     mask_zero_tasks(zl, n, nrb, W, H, pitch, u_out, v_out, out_pitch, valid, det, (blockIdx.x * blockDim.x + threadIdx.x) >> 5,

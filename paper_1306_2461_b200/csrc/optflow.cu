@@ -6,6 +6,7 @@
 #include "../../include/optflow.h"
 #include "of_kernels.cuh"
 #include "of_solve.cuh"
+#include "of_dispatch.cuh"
 #include "of_equalise.cuh"
 #include "of_post.cuh"
 
@@ -133,11 +134,9 @@ template <int R> int setup_attrs()
     CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
 }
 
@@ -241,8 +240,8 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
     a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
     void *args[] = {&a};
-    const void *fn = c->md[0].mask ? (ho ? (const void *)of_solve_pair<R, true, true> : (const void *)of_solve_pair<R, true, false>)
-                                   : (ho ? (const void *)of_solve_pair<R, false, true> : (const void *)of_solve_pair<R, false, false>);
+    if (ho) return of_launch_solve_hoisted(R, c->md[0].mask != nullptr, a, c->sms, st);     // compiled in optflow_hoist.cu
+    const void *fn = c->md[0].mask ? (const void *)of_solve_pair<R, true, false> : (const void *)of_solve_pair<R, false, false>;
     return cudaLaunchCooperativeKernel(fn, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
                                        (size_t)K3Geom<R>::SMEM, st);
 }
@@ -277,18 +276,6 @@ int encode_tensor_maps(of_context *c)
     return OF_OK;
 }
 
-#define DISPATCH_R(R_, CALL)                                                                       \
-    switch (R_) {                                                                                  \
-    case 1: { constexpr int R = 1; CALL; } break;   case 2: { constexpr int R = 2; CALL; } break;   \
-    case 3: { constexpr int R = 3; CALL; } break;   case 4: { constexpr int R = 4; CALL; } break;   \
-    case 5: { constexpr int R = 5; CALL; } break;   case 6: { constexpr int R = 6; CALL; } break;   \
-    case 7: { constexpr int R = 7; CALL; } break;   case 8: { constexpr int R = 8; CALL; } break;   \
-    case 9: { constexpr int R = 9; CALL; } break;   case 10: { constexpr int R = 10; CALL; } break; \
-    case 11: { constexpr int R = 11; CALL; } break; case 12: { constexpr int R = 12; CALL; } break; \
-    case 13: { constexpr int R = 13; CALL; } break; case 14: { constexpr int R = 14; CALL; } break; \
-    case 15: { constexpr int R = 15; CALL; } break; case 16: { constexpr int R = 16; CALL; } break; \
-    default: break;                                                                                \
-    }
 
 void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
 {
@@ -726,6 +713,10 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         if (cudaDeviceSynchronize() != cudaSuccess) rc = fail(OF_ERR_CUDA, "memset failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
     if (rc == OF_OK) { DISPATCH_R(window_radius, rc = setup_attrs<R>()); }
+    if (rc == OF_OK) {
+        cudaError_t e = of_setup_attrs_hoisted(window_radius, SMEM_MAX);
+        if (e != cudaSuccess) rc = fail(OF_ERR_CUDA, "cudaFuncSetAttribute (hoisted solve kernel): %s", cudaGetErrorString(e));
+    }
     if (rc == OF_OK) {
         c->sms = prop.multiProcessorCount;
         c->dbg = getenv("OF_KERNEL_DEBUG") ? atoi(getenv("OF_KERNEL_DEBUG")) : 0;

@@ -1,6 +1,7 @@
 // of_dispatch.cuh -- radius dispatch (a run-time window radius selects a template instantiation) and the entry points of the
-// second translation unit.  The hoisted (of_set_hoist) instantiations of the persistent solve kernel are compiled in
-// optflow_hoist.cu, in parallel with optflow.cu: they are half of the build time and share nothing but headers with the rest.
+// other translation units.  The hoisted (of_set_hoist) instantiations of the persistent solve kernel are compiled in
+// optflow_hoist.cu and the masked (of_set_mask) instantiations of K2, K3 and the solve kernel in optflow_mask.cu, in parallel with
+// optflow.cu: together they are two thirds of the build time and share nothing but headers with the rest.
 #pragma once
 #include "of_solve.cuh"
 
@@ -20,3 +21,9 @@
 // optflow_hoist.cu: of_solve_pair<R, mk, true>.  Launch (cooperative, `sms` CTAs) and one-time attribute set-up.
 cudaError_t of_launch_solve_hoisted(int R, bool mk, const SolveArgs &a, int sms, cudaStream_t st);
 cudaError_t of_setup_attrs_hoisted(int R, int smem_max);
+
+// optflow_mask.cu: k2_products_hsum<R, true>, k3_vsum_solve<R, true>, of_solve_pair<R, true, false>.
+void of_launch_k2_masked(int R, const K2Params &p, int grid, int threads, size_t smem, cudaStream_t st);
+void of_launch_k3_masked(int R, const CUtensorMap &tm, const K3Params &p, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t of_launch_solve_masked(int R, const SolveArgs &a, int sms, cudaStream_t st);
+cudaError_t of_setup_attrs_masked(int R, int smem_max);

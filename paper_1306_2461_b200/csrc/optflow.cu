@@ -134,9 +134,6 @@ template <int R> int setup_attrs()
     CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
 }
 
@@ -211,7 +208,7 @@ void launch_k2(const of_context *c, int l, const float *I1, const float *I2, boo
     const MaskDesc &M = c->md[l];
     K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, M.k2_list ? M.k2_n : P.ntiles,
                   c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list, 0};
-    if (M.mask) k2_products_hsum<R, true><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
+    if (M.mask) of_launch_k2_masked(R, p, P.grid, 32 * P.warps, P.smem + 16, st);                   // compiled in optflow_mask.cu
     else k2_products_hsum<R, false><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
 }
 
@@ -222,7 +219,7 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     const K3Plan &P = c->k3[l];
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
                   L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg, c->md[l], nullptr, 0};
-    if (c->md[l].mask) k3_vsum_solve<R, true><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
+    if (c->md[l].mask) of_launch_k3_masked(R, c->tmS[l], p, P.grid, 32 * (P.warps + 1), P.smem, st);
     else k3_vsum_solve<R, false><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
@@ -241,8 +238,8 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
     void *args[] = {&a};
     if (ho) return of_launch_solve_hoisted(R, c->md[0].mask != nullptr, a, c->sms, st);     // compiled in optflow_hoist.cu
-    const void *fn = c->md[0].mask ? (const void *)of_solve_pair<R, true, false> : (const void *)of_solve_pair<R, false, false>;
-    return cudaLaunchCooperativeKernel(fn, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
+    if (c->md[0].mask) return of_launch_solve_masked(R, a, c->sms, st);                              // compiled in optflow_mask.cu
+    return cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, false, false>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
                                        (size_t)K3Geom<R>::SMEM, st);
 }
 
@@ -715,7 +712,8 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     if (rc == OF_OK) { DISPATCH_R(window_radius, rc = setup_attrs<R>()); }
     if (rc == OF_OK) {
         cudaError_t e = of_setup_attrs_hoisted(window_radius, SMEM_MAX);
-        if (e != cudaSuccess) rc = fail(OF_ERR_CUDA, "cudaFuncSetAttribute (hoisted solve kernel): %s", cudaGetErrorString(e));
+        if (e == cudaSuccess) e = of_setup_attrs_masked(window_radius, SMEM_MAX);
+        if (e != cudaSuccess) rc = fail(OF_ERR_CUDA, "cudaFuncSetAttribute (hoisted / masked kernels): %s", cudaGetErrorString(e));
     }
     if (rc == OF_OK) {
         c->sms = prop.multiProcessorCount;

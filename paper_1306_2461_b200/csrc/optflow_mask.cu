@@ -1,0 +1,34 @@
+// optflow_mask.cu -- the of_set_mask instantiations (MK = true) of K2, K3 and the persistent solve kernel as a translation unit of
+// their own: build.py compiles it in parallel with optflow.cu and optflow_hoist.cu.  Nothing but the entry points of of_dispatch.cuh.
+#include "of_dispatch.cuh"
+
+void of_launch_k2_masked(int R_, const K2Params &p, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    DISPATCH_R(R_, (k2_products_hsum<R, true><<<grid, threads, smem, st>>>(p)));
+}
+
+void of_launch_k3_masked(int R_, const CUtensorMap &tm, const K3Params &p, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    DISPATCH_R(R_, (k3_vsum_solve<R, true><<<grid, threads, smem, st>>>(tm, p)));
+}
+
+cudaError_t of_launch_solve_masked(int R_, const SolveArgs &a, int sms, cudaStream_t st)
+{
+    cudaError_t e = cudaErrorInvalidValue;
+    SolveArgs args_copy = a;
+    void *args[] = {&args_copy};
+    DISPATCH_R(R_, e = cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, true, false>, dim3(sms), dim3(32 * SOLVE_WARPS), args,
+                                                   (size_t)K3Geom<R>::SMEM, st));
+    return e;
+}
+
+cudaError_t of_setup_attrs_masked(int R_, int smem_max)
+{
+    cudaError_t e = cudaErrorInvalidValue;
+    DISPATCH_R(R_, {
+        e = cudaFuncSetAttribute(k2_products_hsum<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k3_vsum_solve<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(of_solve_pair<R, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+    });
+    return e;
+}

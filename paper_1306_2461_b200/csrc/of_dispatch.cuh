@@ -18,9 +18,12 @@
     default: break;                                                                                \
     }
 
-// optflow_hoist.cu: of_solve_pair<R, mk, true>.  Launch (cooperative, `sms` CTAs) and one-time attribute set-up.
+// optflow_hoist.cu: of_solve_pair<R, false, true>; forwards to optflow_hoist_mask.cu (of_solve_pair<R, true, true>) when mk is set.
+// Launch (cooperative, `sms` CTAs) and one-time attribute set-up (both units).
 cudaError_t of_launch_solve_hoisted(int R, bool mk, const SolveArgs &a, int sms, cudaStream_t st);
 cudaError_t of_setup_attrs_hoisted(int R, int smem_max);
+cudaError_t of_launch_solve_hoisted_masked(int R, const SolveArgs &a, int sms, cudaStream_t st);
+cudaError_t of_setup_attrs_hoisted_masked(int R, int smem_max);
 
 // optflow_mask.cu: k2_products_hsum<R, true>, k3_vsum_solve<R, true>, of_solve_pair<R, true, false>.
 void of_launch_k2_masked(int R, const K2Params &p, int grid, int threads, size_t smem, cudaStream_t st);

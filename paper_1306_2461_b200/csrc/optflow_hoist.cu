@@ -1,23 +1,23 @@
-// optflow_hoist.cu -- the of_set_hoist instantiations of the persistent solve kernel, of_solve_pair<R, MK, true> (of_solve.cuh), as a
-// translation unit of their own: build.py compiles it in parallel with optflow.cu.  Nothing but the two entry points below.
+// optflow_hoist.cu -- the of_set_hoist instantiations of the persistent solve kernel without a mask, of_solve_pair<R, false, true>
+// (of_solve.cuh), as a translation unit of their own: build.py compiles it in parallel with the others.  The masked ones,
+// of_solve_pair<R, true, true>, are in optflow_hoist_mask.cu.  Nothing but the entry points of of_dispatch.cuh.
 #include "of_dispatch.cuh"
 
 cudaError_t of_launch_solve_hoisted(int R_, bool mk, const SolveArgs &a, int sms, cudaStream_t st)
 {
+    if (mk) return of_launch_solve_hoisted_masked(R_, a, sms, st);
     cudaError_t e = cudaErrorInvalidValue;
     SolveArgs args_copy = a;
     void *args[] = {&args_copy};
-    DISPATCH_R(R_, e = cudaLaunchCooperativeKernel(mk ? (const void *)of_solve_pair<R, true, true> : (const void *)of_solve_pair<R, false, true>,
-                                                   dim3(sms), dim3(32 * SOLVE_WARPS), args, (size_t)K3Geom<R>::SMEM, st));
+    DISPATCH_R(R_, e = cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, false, true>, dim3(sms), dim3(32 * SOLVE_WARPS), args,
+                                                   (size_t)K3Geom<R>::SMEM, st));
     return e;
 }
 
 cudaError_t of_setup_attrs_hoisted(int R_, int smem_max)
 {
     cudaError_t e = cudaErrorInvalidValue;
-    DISPATCH_R(R_, {
-        e = cudaFuncSetAttribute(of_solve_pair<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(of_solve_pair<R, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
-    });
+    DISPATCH_R(R_, e = cudaFuncSetAttribute(of_solve_pair<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max));
+    if (e == cudaSuccess) e = of_setup_attrs_hoisted_masked(R_, smem_max);
     return e;
 }

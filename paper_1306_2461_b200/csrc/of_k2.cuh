@@ -133,14 +133,6 @@ __device__ __forceinline__ K2Tap k2_gather(const float *__restrict__ I2, float x
     return t;
 }
 
-__device__ __forceinline__ float k2_lerp(const K2Tap &t)
-{
-    const float bx = 1.0f - t.ax, by = 1.0f - t.ay;
-    const float top = fmaf(t.ax, t.i01, bx * t.i00);
-    const float bot = fmaf(t.ax, t.i11, bx * t.i10);
-    return fmaf(t.ay, bot, by * top);
-}
-
 // The four pixels of one phase-1 task: gathers first (k2_task_gather), products later (k2_task_products).
 __device__ __forceinline__ void k2_task_gather(const K2Params &p, const K2In &in, int x, int y, K2Tap (&t)[4])
 {
@@ -151,13 +143,27 @@ __device__ __forceinline__ void k2_task_gather(const K2Params &p, const K2In &in
     t[3] = k2_gather(p.I2, xf + 1.0f, yf + 1.0f, Wm2f, Hm2f, p.pitch, in.u1.y, in.v1.y);
 }
 
-// It = I2w - I1 - Ix*u - Iy*v (D10) and the five products.  gx, gy are already multiplied by the
-// validity mask (0 outside the image -> all five products are zero, D12).
-__device__ __forceinline__ void k2_products(float I2w, float uu, float vv, float c, float gx, float gy,
-                                            float &xx, float &xy, float &yy, float &xt, float &yt)
+// It = I2w - I1 - Ix*u - Iy*v (D10) and the five products of the four pixels of a task, two pixels (rows y, y+1 of one column) per
+// packed fp32 instruction (FADD2 / FMUL2 / FFMA2: every component is rounded exactly like the scalar instruction, so the values do
+// not depend on the packing).  gx, gy are already multiplied by the validity mask (0 outside the image -> all five products are
+// zero, D12).
+__device__ __forceinline__ float2 k2_lerp2(const K2Tap &a, const K2Tap &b)
 {
-    const float It = fmaf(-gy, vv, fmaf(-gx, uu, I2w - c));
-    xx = gx * gx; xy = gx * gy; yy = gy * gy; xt = gx * It; yt = gy * It;
+    const float2 one = make_float2(1.0f, 1.0f);
+    const float2 ax = make_float2(a.ax, b.ax), ay = make_float2(a.ay, b.ay);
+    const float2 bx = __fadd2_rn(one, make_float2(-a.ax, -b.ax)), by = __fadd2_rn(one, make_float2(-a.ay, -b.ay));
+    const float2 top = __ffma2_rn(ax, make_float2(a.i01, b.i01), __fmul2_rn(bx, make_float2(a.i00, b.i00)));
+    const float2 bot = __ffma2_rn(ax, make_float2(a.i11, b.i11), __fmul2_rn(bx, make_float2(a.i10, b.i10)));
+    return __ffma2_rn(ay, bot, __fmul2_rn(by, top));
+}
+
+// one column of a task: pixels (x, y) and (x, y+1)
+__device__ __forceinline__ void k2_products2(float2 I2w, float2 uu, float2 vv, float2 c, float2 gx, float2 gy,
+                                             float2 &xx, float2 &xy, float2 &yy, float2 &xt, float2 &yt)
+{
+    const float2 ngx = make_float2(-gx.x, -gx.y), ngy = make_float2(-gy.x, -gy.y);
+    const float2 It = __ffma2_rn(ngy, vv, __ffma2_rn(ngx, uu, __fadd2_rn(I2w, make_float2(-c.x, -c.y))));
+    xx = __fmul2_rn(gx, gx); xy = __fmul2_rn(gx, gy); yy = __fmul2_rn(gy, gy); xt = __fmul2_rn(gx, It); yt = __fmul2_rn(gy, It);
 }
 
 template <bool MK> __device__ __forceinline__ void k2_task_products(const K2Params &p, const K2In &cur, int x, int y, const K2Tap (&t)[4], float4 (&o)[5])
@@ -168,14 +174,20 @@ template <bool MK> __device__ __forceinline__ void k2_task_products(const K2Para
         m00 = (cur.m0 & 0xffu) ? m00 : 0.f; m01 = (cur.m0 >> 8) ? m01 : 0.f;
         m10 = (cur.m1 & 0xffu) ? m10 : 0.f; m11 = (cur.m1 >> 8) ? m11 : 0.f;
     }
-    k2_products(k2_lerp(t[0]), cur.u0.x, cur.v0.x, cur.c0.x, m00 * ((in1 ? cur.c0.y : cur.c0.x) - cur.l0), m00 * (cur.c1.x - cur.cm.x),
-                o[0].x, o[1].x, o[2].x, o[3].x, o[4].x);
-    k2_products(k2_lerp(t[1]), cur.u1.x, cur.v1.x, cur.c1.x, m10 * ((in1 ? cur.c1.y : cur.c1.x) - cur.l1), m10 * (cur.c2.x - cur.c0.x),
-                o[0].y, o[1].y, o[2].y, o[3].y, o[4].y);
-    k2_products(k2_lerp(t[2]), cur.u0.y, cur.v0.y, cur.c0.y, m01 * (cur.q0 - cur.c0.x), m01 * (cur.c1.y - cur.cm.y),
-                o[0].z, o[1].z, o[2].z, o[3].z, o[4].z);
-    k2_products(k2_lerp(t[3]), cur.u1.y, cur.v1.y, cur.c1.y, m11 * (cur.q1 - cur.c1.x), m11 * (cur.c2.y - cur.c0.y),
-                o[0].w, o[1].w, o[2].w, o[3].w, o[4].w);
+    // column x (rows y, y+1), then column x+1
+    const float2 ma = make_float2(m00, m10), mb = make_float2(m01, m11);
+    const float2 rgt_a = make_float2(in1 ? cur.c0.y : cur.c0.x, in1 ? cur.c1.y : cur.c1.x);
+    const float2 gxa = __fmul2_rn(ma, __fadd2_rn(rgt_a, make_float2(-cur.l0, -cur.l1)));
+    const float2 gya = __fmul2_rn(ma, __fadd2_rn(make_float2(cur.c1.x, cur.c2.x), make_float2(-cur.cm.x, -cur.c0.x)));
+    const float2 gxb = __fmul2_rn(mb, __fadd2_rn(make_float2(cur.q0, cur.q1), make_float2(-cur.c0.x, -cur.c1.x)));
+    const float2 gyb = __fmul2_rn(mb, __fadd2_rn(make_float2(cur.c1.y, cur.c2.y), make_float2(-cur.cm.y, -cur.c0.y)));
+    float2 xx, xy, yy, xt, yt;
+    k2_products2(k2_lerp2(t[0], t[1]), make_float2(cur.u0.x, cur.u1.x), make_float2(cur.v0.x, cur.v1.x), make_float2(cur.c0.x, cur.c1.x), gxa, gya,
+                 xx, xy, yy, xt, yt);
+    o[0].x = xx.x; o[0].y = xx.y; o[1].x = xy.x; o[1].y = xy.y; o[2].x = yy.x; o[2].y = yy.y; o[3].x = xt.x; o[3].y = xt.y; o[4].x = yt.x; o[4].y = yt.y;
+    k2_products2(k2_lerp2(t[2], t[3]), make_float2(cur.u0.y, cur.u1.y), make_float2(cur.v0.y, cur.v1.y), make_float2(cur.c0.y, cur.c1.y), gxb, gyb,
+                 xx, xy, yy, xt, yt);
+    o[0].z = xx.x; o[0].w = xx.y; o[1].z = xy.x; o[1].w = xy.y; o[2].z = yy.x; o[2].w = yy.y; o[3].z = xt.x; o[3].w = xt.y; o[4].z = yt.x; o[4].w = yt.y;
 }
 
 // One K2 pass over a level by one CTA: it owns the contiguous range [t_begin, t_end) of warp tiles

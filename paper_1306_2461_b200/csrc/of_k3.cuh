@@ -8,9 +8,9 @@
 //     64 x K3_SEG x 5 floats (5 KB) fetched by a single cp.async.bulk.tensor into a shared-memory ring;
 //     rows above/below the image are zero-filled by the TMA unit, which IS the zero extension of the
 //     window (D12) -- no border code;
-//   * one PRODUCER warp walks the CTA's chunks in order: waits for the ring slot to be released
-//     (empty mbarrier, NC arrivals = the NC tasks that read a chunk), arms the full mbarrier with
-//     expect_tx and issues the TMA; when its last chunk is issued it joins the consumers;
+//   * one PRODUCER warp issues the CTA's chunks, its 32 lanes in parallel (a lane needs ~105 cycles per copy): each waits for
+//     the ring slot to be released (empty mbarrier, NC arrivals = the NC tasks that read a chunk), arms the full mbarrier
+//     with expect_tx and issues the TMA; when its last chunk is issued the warp joins the consumers;
 //   * the CONSUMER warps (K3_MAX_NW = 11) pull tasks from a shared-memory counter (balances the four SM
 //     sub-partitions), wait on the full barriers of their NC chunks, sum, release the chunks, solve.
 //     No __syncthreads after set-up.  Which warp runs a task does not change its arithmetic, so the
@@ -21,7 +21,7 @@
 // Direct (2R+1)-tap sums, fixed order, no atomics on data: no cancellation (H2).
 #pragma once
 #include "of_common.cuh"
-#include <cuda.h>
+#include "of_async.cuh"
 
 #ifndef K3_SEG
 #define K3_SEG 4                                          // rows per task = rows per TMA chunk (4: finer tasks, better
@@ -32,7 +32,7 @@
 #define K3_MAX_NW 11                                      // consumer warps (+1 producer warp)
 #endif
 #ifndef K3_RING
-#define K3_RING (176 / K3_SEG)                            // chunks in the ring (220 KB)
+#define K3_RING (176 / K3_SEG)                            // chunks in the ring (220 KB); must exceed 32 (see the producer)
 #endif
 
 template <int R> struct K3Geom {
@@ -58,36 +58,6 @@ struct K3Params {
     float *G;                        // of_set_hoist: three planes (stride `gplane`, pitch `pitch`) holding the window sums a, b, c
     size_t gplane;                   //   of IxIx, IxIy, IyIy of the level (written by an HM = 1 pass, read by HM = 2 passes)
 };
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *tm, int x, int y, int z, uint32_t bar)
-{
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-                 ::"r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(bar) : "memory");
-}
 
 // a - b on a pair with one packed instruction
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return fma2s(-1.0f, b, a); }
@@ -174,19 +144,28 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
     // Task i of this CTA (global task t_begin+i in strip s) reads ring chunks gc0 + i + (s-s_first)*(NC-1) + k.
 
     if (warp == NWC) {
-        // ===================== producer: one lane walks the chunks of every segment in order
-        if (lane == 0 && !(p.dbg & 1)) {
+        // ===================== producer: the 32 lanes share the chunks of every run (lane k issues chunks k, k + 32, ...).
+        // One lane needs ~105 cycles per bulk tensor copy (expect_tx + issue; measured, profiles/r2_tma_issue.md), so a single
+        // lane delivered the ~40 chunks of a level-0 pass only after ~6700 cycles; 32 lanes have them in flight after ~2300.
+        // Consumers wait on the full barrier of each chunk, so the order of issue does not matter.
+        if (!(p.dbg & 1)) {
             // one run = `ntask` consecutive tasks of strip s from row block rb0; its chunks start at ring chunk gbase
             auto produce_run = [&](int s, int rb0, int ntask, int gbase) {
                 const int total = ntask + NC - 1;
                 const int x0 = 64 * s, yc0 = K3_SEG * rb0 - R;          // chunk c holds rows yc0 + K3_SEG*c ...
-                for (int c = 0; c < total; ++c) {
-                    const int gc = gbase + c, slot = gc % K3_RING, use = gc / K3_RING;
-                    if (use > 0) mbar_wait(empty0 + 8 * slot, (use - 1) & 1);
-                    const int readers = min(ntask - 1, c) - max(0, c - NC + 1) + 1;
-                    if (readers < NC) mbar_arrive(empty0 + 8 * slot, NC - readers);   // stand-ins for tasks that do not exist
-                    mbar_expect_tx(full0 + 8 * slot, CHUNK_TX);
-                    tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + K3_SEG * c, F0, full0 + 8 * slot);
+                // batches of 32 chunks with a warp barrier in between: two uses of one ring slot are K3_RING > 32 chunks apart,
+                // so no lane can wait for a slot's release two uses ahead (an mbarrier only tells the parity of its phase)
+                for (int c0 = 0; c0 < total; c0 += 32) {
+                    const int c = c0 + lane;
+                    if (c < total) {
+                        const int gc = gbase + c, slot = gc % K3_RING, use = gc / K3_RING;
+                        if (use > 0) mbar_wait(empty0 + 8 * slot, (use - 1) & 1);
+                        const int readers = min(ntask - 1, c) - max(0, c - NC + 1) + 1;
+                        if (readers < NC) mbar_arrive(empty0 + 8 * slot, NC - readers);   // stand-ins for tasks that do not exist
+                        mbar_expect_tx(full0 + 8 * slot, CHUNK_TX);
+                        tma_load_3d(ring0 + slot * K3_CHUNK_BYTES, tmS, x0, yc0 + K3_SEG * c, F0, full0 + 8 * slot);
+                    }
+                    __syncwarp();
                 }
             };
             if (MK) {                                                   // compacted lists: the host has cut the runs

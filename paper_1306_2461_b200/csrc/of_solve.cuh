@@ -18,7 +18,17 @@
 //     after the K2 pass orders its generic-proxy stores before the TMA writes of the K3 pass.
 #pragma once
 #include "of_k2.cuh"
+#include "of_k2s.cuh"
 #include "of_k3.cuh"
+
+// K2 variant of the unmasked kernels: 0 (default) = warp tiles with global gathers (of_k2.cuh), 1 (-DOF_K2_STREAMING) = the
+// task-queue form with the TMA-staged I2 window (of_k2s.cuh).  Both are kept bit-identical; profiles/r2_k2_streaming.md has the
+// measurements that decided the default.
+#ifdef OF_K2_STREAMING
+#define SOLVE_K2S 1
+#else
+#define SOLVE_K2S 0
+#endif
 
 #define SOLVE_TIMELINE_MAX 4096
 #ifndef SOLVE_WARPS
@@ -29,8 +39,19 @@ struct LevelDesc {
     const float *pyr[2];                     // pyramid slots (I1 / I2 chosen per job)
     float *u, *v;
     int W, H, pitch;
-    int k2_nseg, k2_nrp, k2_tiles_y, k2_ntiles;
+    int k2_nseg, k2_nrp, k2_tiles_y, k2_ntiles;   // warp tiles of of_k2.cuh (masked instantiations)
     int k3_nrb, k3_ntasks;
+    int k2s_nuy, k2s_nunits;                 // units of of_k2s.cuh: per strip, per level
+    unsigned long long k2s_magic;            // ceil(2^40 / k2s_nuy)
+};
+
+// Dynamic shared memory of the solve kernel: [0, 225280) data (K3 ring / K2 product buffers, A slots and I2 ring), then the K3
+// barriers and counters (720 B), then the K2 barriers, descriptors and ticket counter.
+#define SOLVE_K2S_BAR_OFF (K3_RING * K3_CHUNK_BYTES + 768)
+template <int R> struct SolveSmem {
+    static constexpr int BYTES = SOLVE_K2S_BAR_OFF + K2S<R>::BAR_BYTES;
+    static_assert(K3Geom<R>::SMEM <= SOLVE_K2S_BAR_OFF && K2S<R>::DATA_BYTES <= K3_RING * K3_CHUNK_BYTES && K2S<R>::DATA_MAX == K3_RING * K3_CHUNK_BYTES,
+                  "shared-memory map of the solve kernel");
 };
 
 #define SOLVE_MAX_LEVELS 12
@@ -48,6 +69,7 @@ struct SolveArgs {
     unsigned long long *prof;                // optional timelines [ncta][SOLVE_TIMELINE_MAX] (SM clock at every phase boundary) or NULL
     WinWeights ww;
     SolveParams sp;
+    const K2SMaps *k2maps;                   // device array [levels]: tensor maps of the K2 inputs (of_k2s.cuh)
     const MaskDesc *md;                      // device array [levels]: obstacle masks and work lists (read by the MK kernel only;
                                              // last, so that every other field keeps its place in the parameter bank)
     // of_set_hoist (HO instantiation only): the planes IxIt, IyIt of a level as an (x, y, field) tensor with a two-field
@@ -73,7 +95,13 @@ __device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned ncta, unsig
     if (threadIdx.x == 0) {
         const unsigned target = (k + 1) * ncta;
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+#ifdef OF_WATCHDOG
+        const long long t0 = clock64();
+        while (ld_acquire_u32(bar) < target)
+            if (clock64() - t0 > 2000000000ll) { printf("[optflow watchdog] block %d: grid barrier %u never completed\n", blockIdx.x, k); __trap(); }
+#else
         while (ld_acquire_u32(bar) < target) { }
+#endif
     }
     ++k;
     __syncthreads();
@@ -185,10 +213,15 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int cta = blockIdx.x, ncta = gridDim.x;
     const K3Smem sm(solve_smem);
-    if (threadIdx.x == 0) k3_init_barriers<R>(sm);
+    const K2SSmem<R> sm2(solve_smem, solve_smem + SOLVE_K2S_BAR_OFF);
+    if (threadIdx.x == 0) {
+        if (SOLVE_K2S && !MK) k2s_init_barriers<R>(sm2);
+        k3_init_barriers<R>(sm);
+    }
     __syncthreads();
 
     uint32_t gc0 = 0;                                            // ring chunks consumed so far by this CTA
+    uint32_t uk0 = 0;                                            // K2 units processed so far by this CTA
     unsigned nbar = 0;                                           // grid barriers passed so far
     int pi = 0;
     prof_stamp(a, pi);
@@ -207,7 +240,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             prof_stamp(a, pi);
         }
         int k2_b, k2_e, k3_b, k3_e;                              // this CTA's share of the level's tiles and tasks
-        cta_range(MK ? M.k2_n : L.k2_ntiles, cta, ncta, k2_b, k2_e);
+        cta_range(MK ? M.k2_n : (SOLVE_K2S ? L.k2s_nunits : L.k2_ntiles), cta, ncta, k2_b, k2_e);
         cta_range(L.k3_ntasks, cta, ncta, k3_b, k3_e);
         uint32_t k3_chunks = (uint32_t)k3_cta_chunks<R>(k3_b, k3_e, L.k3_nrb);
         if (MK) {                                                // mask set: the host has cut the compacted task list per CTA
@@ -216,11 +249,18 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
         }
         K2Params p2 = {L.pyr[a.s1], L.pyr[a.s2], L.u, L.v, a.S, a.plane, L.W, L.H, L.pitch,
                        L.k2_nseg, L.k2_nrp, L.k2_tiles_y, L.k2_ntiles, a.ww, 0, a.dbg, M.mask, M.k2_list, 0};
+        K2SParams q2 = {a.k2maps + l, a.s2, L.pyr[a.s1], L.pyr[a.s2], L.u, L.v, a.S, a.plane, L.W, L.H, L.pitch, L.k2s_nuy, L.k2s_nunits, L.k2s_magic, a.ww, 0, 0};
         for (int it = 0; it < a.iterations; ++it) {
             // ---- K2 pass: warp + gradients + products + horizontal sums -> five planes
             p2.zero_uv = (l == top && it == 0) ? 1 : 0;            // zero initial guess at the coarsest level
             p2.f_first = (HO && it > 0) ? 3 : 0;
-            k2_phase<R, MK, HO>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
+            if constexpr (MK || !SOLVE_K2S) {
+                k2_phase<R, MK, HO>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
+            } else {
+                q2.zero_uv = p2.zero_uv; q2.f_first = p2.f_first;
+                k2s_phase<R, HO>(q2, sm2, warp, lane, k2_b, k2_e, uk0);
+                uk0 += (uint32_t)(k2_e - k2_b);
+            }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             prof_stamp(a, pi);
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
@@ -234,6 +274,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             else if (it == 0) k3_phase<R, MK, 1>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
             else k3_phase<R, MK, 2>(&a.tm2[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
             gc0 += k3_chunks;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the ring was read by generic loads; the next K2 pass copies into it
             __syncthreads();
             if (threadIdx.x == 0) { sm.counter[0] = 0; sm.counter[1] = 0; }
             prof_stamp(a, pi);

@@ -101,6 +101,8 @@ struct of_context {
     K2Plan k2[OF_MAX_LEVELS];
     K3Plan k3[OF_MAX_LEVELS];
     CUtensorMap tmS[OF_MAX_LEVELS];     // the five summed planes of a level as one (x, y, field) tensor
+    K2SMaps *d_k2maps;                  // tensor maps of the K2 inputs per level (of_k2s.cuh), device array
+    int k2s_nuy[OF_MAX_LEVELS], k2s_nunits[OF_MAX_LEVELS];
     LevelDesc *d_lv;                    // device copies for the persistent solve kernel
     MaskDesc *d_md;
     CUtensorMap *d_tm;
@@ -128,10 +130,15 @@ struct of_context {
 namespace {
 
 inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
+inline unsigned long long k2s_magic(int nuy) { return ((1ull << 40) + (unsigned long long)nuy - 1) / (unsigned long long)nuy; }
 
 template <int R> int setup_attrs()
 {
+#if SOLVE_K2S
+    CU_TRY(cudaFuncSetAttribute(k2s_products_hsum<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+#else
     CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+#endif
     CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
@@ -198,6 +205,8 @@ template <int R> void plan_level(of_context *c, int l)
 {
     c->k2[l] = plan_k2<R>(c->lv[l].W, c->lv[l].H, c->sms);
     c->k3[l] = plan_k3<R>(c->lv[l].W, c->lv[l].H, c->sms);
+    c->k2s_nuy[l] = (c->lv[l].H + K2S<R>::RU - 1) / K2S<R>::RU;
+    c->k2s_nunits[l] = ((c->lv[l].W + K2S<R>::TW - 1) / K2S<R>::TW) * c->k2s_nuy[l];
 }
 
 template <int R>
@@ -208,8 +217,14 @@ void launch_k2(const of_context *c, int l, const float *I1, const float *I2, boo
     const MaskDesc &M = c->md[l];
     K2Params p = {I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, P.nseg, P.nrp, P.tiles_y, M.k2_list ? M.k2_n : P.ntiles,
                   c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list, 0};
-    if (M.mask) of_launch_k2_masked(R, p, P.grid, 32 * P.warps, P.smem + 16, st);                   // compiled in optflow_mask.cu
-    else k2_products_hsum<R, false><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
+    if (M.mask) { of_launch_k2_masked(R, p, P.grid, 32 * P.warps, P.smem + 16, st); return; }    // compiled in optflow_mask.cu
+#if !SOLVE_K2S
+    k2_products_hsum<R, false><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
+#else
+    const int s2 = I2 == c->pyr[1][l] ? 1 : 0;
+    K2SParams q = {c->d_k2maps + l, s2, I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, c->k2s_nuy[l], c->k2s_nunits[l], k2s_magic(c->k2s_nuy[l]), c->ww, zero_uv ? 1 : 0, 0};
+    k2s_products_hsum<R><<<c->sms, 32 * (K2S_WORKERS + 1), K2S<R>::DATA_MAX + K2S<R>::BAR_BYTES, st>>>(q);
+#endif
 }
 
 template <int R>
@@ -231,7 +246,7 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
     a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
     a.valid = c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
-    a.md = c->d_md; a.G = c->G;
+    a.md = c->d_md; a.G = c->G; a.k2maps = c->d_k2maps;
     const bool ho = c->hoist && c->G != nullptr;
     if (ho) memcpy(a.tm2, c->tmS2, sizeof(CUtensorMap) * c->levels);
     a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
@@ -240,7 +255,31 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     if (ho) return of_launch_solve_hoisted(R, c->md[0].mask != nullptr, a, c->sms, st);     // compiled in optflow_hoist.cu
     if (c->md[0].mask) return of_launch_solve_masked(R, a, c->sms, st);                              // compiled in optflow_mask.cu
     return cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, false, false>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
-                                       (size_t)K3Geom<R>::SMEM, st);
+                                       (size_t)SolveSmem<R>::BYTES, st);
+}
+
+// Tensor maps of the staged K2 input (of_k2s.cuh): per level the two pyramid slots as I2, box = one group of window rows.
+template <int R> int encode_k2s_maps(of_context *c, void *fn)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    typedef K2S<R> G;
+    std::vector<K2SMaps> maps(c->levels);
+    for (int l = 0; l < c->levels; ++l) {
+        const Level &L = c->lv[l];
+        cuuint64_t dims[2] = {(cuuint64_t)L.pitch, (cuuint64_t)L.H};
+        cuuint64_t strides[1] = {(cuuint64_t)L.pitch * sizeof(float)};
+        cuuint32_t box[2] = {G::PWB, G::RU};
+        cuuint32_t estr[2] = {1, 1};
+        for (int s = 0; s < N_PYR; ++s) {
+            CUresult r = ((encode_fn)fn)(&maps[l].i2[s], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, c->pyr[s][l], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return fail(OF_ERR_CUDA, "cuTensorMapEncodeTiled(I2 window, level %d) failed: CUresult %d", l, (int)r);
+        }
+    }
+    CU_TRY(cudaMemcpy(c->d_k2maps, maps.data(), sizeof(K2SMaps) * c->levels, cudaMemcpyHostToDevice));
+    return OF_OK;
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency:
@@ -254,6 +293,11 @@ int encode_tensor_maps(of_context *c)
     cudaDriverEntryPointQueryResult qres;
     CU_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
     if (!fn || qres != cudaDriverEntryPointSuccess) return fail(OF_ERR_CUDA, "cuTensorMapEncodeTiled is not available in this driver");
+    {
+        int rc = OF_OK;
+        DISPATCH_R(c->R, rc = encode_k2s_maps<R>(c, fn));
+        if (rc != OF_OK) return rc;
+    }
     for (int l = 0; l < c->levels; ++l) {
         const Level &L = c->lv[l];
         cuuint64_t dims[3] = {(cuuint64_t)L.pitch, (cuuint64_t)L.H, 5};
@@ -571,7 +615,8 @@ int upload_level_descs(of_context *c)
     LevelDesc hl[OF_MAX_LEVELS];
     for (int l = 0; l < c->levels; ++l)
         hl[l] = {{c->pyr[0][l], c->pyr[1][l]}, c->u[l], c->v[l], c->lv[l].W, c->lv[l].H, c->lv[l].pitch,
-                 c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks};
+                 c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks,
+                 c->k2s_nuy[l], c->k2s_nunits[l], k2s_magic(c->k2s_nuy[l])};
     CU_TRY(cudaMemcpy(c->d_lv, hl, sizeof(LevelDesc) * c->levels, cudaMemcpyHostToDevice));
     CU_TRY(cudaMemcpy(c->d_md, c->md, sizeof(MaskDesc) * c->levels, cudaMemcpyHostToDevice));
     return OF_OK;
@@ -688,8 +733,8 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     for (int l = 0; l < levels && rc == OF_OK; ++l) {
         size_t bytes = sizeof(float) * (size_t)lv[l].pitch * lv[l].H;
         for (int s = 0; s < N_PYR && rc == OF_OK; ++s) rc = dev_alloc(c, (void **)&c->pyr[s][l], bytes);
-        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->u[l], bytes);
-        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->v[l], bytes);
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->u[l], 2 * bytes);      // u then v: one (x, y, {u, v}) tensor for the K2 copies
+        if (rc == OF_OK) c->v[l] = c->u[l] + (size_t)lv[l].pitch * lv[l].H;
     }
     c->plane = (size_t)lv[0].pitch * lv[0].H;
     if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->S, sizeof(float) * 5 * c->plane);
@@ -719,7 +764,8 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         c->sms = prop.multiProcessorCount;
         c->dbg = getenv("OF_KERNEL_DEBUG") ? atoi(getenv("OF_KERNEL_DEBUG")) : 0;
         for (int l = 0; l < levels; ++l) { DISPATCH_R(window_radius, plan_level<R>(c, l)); }
-        rc = encode_tensor_maps(c);
+        rc = dev_alloc(c, (void **)&c->d_k2maps, sizeof(K2SMaps) * levels);
+        if (rc == OF_OK) rc = encode_tensor_maps(c);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_lv, sizeof(LevelDesc) * levels);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_md, sizeof(MaskDesc) * OF_MAX_LEVELS);
         if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->d_tm, sizeof(CUtensorMap) * levels);

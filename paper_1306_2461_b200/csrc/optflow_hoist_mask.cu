@@ -7,7 +7,7 @@ cudaError_t of_launch_solve_hoisted_masked(int R_, const SolveArgs &a, int sms, 
     SolveArgs args_copy = a;
     void *args[] = {&args_copy};
     DISPATCH_R(R_, e = cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, true, true>, dim3(sms), dim3(32 * SOLVE_WARPS), args,
-                                                   (size_t)K3Geom<R>::SMEM, st));
+                                                   (size_t)SolveSmem<R>::BYTES, st));
     return e;
 }
 

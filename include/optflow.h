@@ -107,6 +107,14 @@ int of_set_graph(of_handle h, int enable);
  * launch.  Both give bit-identical results. */
 int of_set_persistent(of_handle h, int enable);
 
+/* Iterate the coarse pyramid levels in fused form (default on; "coarse-to-fine": a further level
+ * should cost ~2 %).  At a level whose image can be cut into at most one tile per SM that fits in shared memory together with its
+ * window halo, a CTA forms the products, both window sums and the solve of its tile without leaving the SM and the field is double
+ * buffered, so an iteration needs one grid barrier instead of two and the five summed planes of that level stay in shared memory.
+ * Every value is formed by the same instructions as in the two-pass form: results are bit-identical with 0 and with
+ * of_set_persistent(h, 0).  Levels with an obstacle mask keep the two-pass form.  Synchronises the device (a set-up call). */
+int of_set_fused(of_handle h, int enable);
+
 /* Hoist what does not change within a pyramid level out of its iterations (default off).  Ix, Iy are
  * differences of I1 alone (reading D9 of DESIGN.md), so the planes IxIx, IxIy, IyIy -- and their
  * window sums, the 2x2 matrix of the paper's local least-squares problem, PAPER.md:59-63 -- are the

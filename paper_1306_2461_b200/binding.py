@@ -34,6 +34,7 @@ SIGNATURES = {
     "of_set_graph": (_i, [_vp, _i]),
     "of_set_persistent": (_i, [_vp, _i]),
     "of_set_hoist": (_i, [_vp, _i]),
+    "of_set_fused": (_i, [_vp, _i]),
     "of_solve_timeline": (_i, [_vp, _i, _i, _vp, _i]),
     "of_get_validity": (_i, [_vp, _vp, _vp]),
     "of_level_size": (_i, [_vp, _i, _c.POINTER(_i), _c.POINTER(_i)]),
@@ -169,6 +170,9 @@ class OpticalFlow:
 
     def set_persistent(self, enable: bool):
         _check(lib().of_set_persistent(self._h, 1 if enable else 0))
+
+    def set_fused(self, enable: bool):
+        _check(lib().of_set_fused(self._h, 1 if enable else 0))
 
     def set_hoist(self, enable: bool):
         _check(lib().of_set_hoist(self._h, 1 if enable else 0))

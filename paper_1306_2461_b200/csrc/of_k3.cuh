@@ -89,6 +89,51 @@ __device__ __forceinline__ void k3_solve_pair(float2 a, float2 b, float2 c, floa
     dv.y = tr.y > 0.f ? fminf(fmaxf(dv.y, -ms), ms) : 0.f;
 }
 
+// Damped 2x2 solve, clamp, update and stores of one task (K3_SEG rows x 2 columns per lane) from its five window sums.  Shared by
+// the K3 pass and the fused coarse-level pass (of_fused.cuh), so both form every value with the same instructions.
+template <bool MK, int SEG = K3_SEG>
+__device__ __forceinline__ void k3_solve_store(const K3Params &p, const float2 (&acc)[5][SEG], const float2 (&uu)[SEG], const float2 (&vv)[SEG],
+                                               const unsigned (&mk)[SEG], int gx, int gy0, int nrows)
+{
+    const int W = p.W, pitch = p.pitch;
+    // ---- solve + update for K3_SEG rows x 2 columns
+    const bool pair_ok = gx + 1 < W;
+    const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
+    float *uo = p.u_out + (size_t)gy0 * p.out_pitch + gx, *vo = p.v_out + (size_t)gy0 * p.out_pitch + gx;
+    float2 trs[SEG], dets[SEG];
+#pragma unroll
+    for (int j = 0; j < SEG; ++j) {
+        float2 du, dv;
+        k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, trs[j], dets[j]);
+        float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
+        if (MK) {                                    // M3: no vector over an obstacle
+            if (!(mk[j] & 0xffu)) { un.x = 0.f; vn.x = 0.f; trs[j].x = 0.f; dets[j].x = 0.f; }
+            if (!(mk[j] >> 8)) { un.y = 0.f; vn.y = 0.f; trs[j].y = 0.f; dets[j].y = 0.f; }
+        }
+        if (j < nrows) {
+            if (vec_out) {
+                *reinterpret_cast<float2 *>(uo + j * p.out_pitch) = un;
+                *reinterpret_cast<float2 *>(vo + j * p.out_pitch) = vn;
+            } else {
+                uo[j * p.out_pitch] = un.x; vo[j * p.out_pitch] = vn.x;
+                if (pair_ok) { uo[j * p.out_pitch + 1] = un.y; vo[j * p.out_pitch + 1] = vn.y; }
+            }
+        }
+    }
+    if (p.valid) {                                   // last iteration of level 0 only
+        uint8_t *m = p.valid + (size_t)gy0 * W + gx;
+        float *d = p.det + (size_t)gy0 * pitch + gx;
+#pragma unroll
+        for (int j = 0; j < SEG; ++j) {
+            if (j < nrows) {
+                m[j * W] = trs[j].x > 0.f ? 1 : 0;
+                d[j * pitch] = dets[j].x;
+                if (pair_ok) { m[j * W + 1] = trs[j].y > 0.f ? 1 : 0; d[j * pitch + 1] = dets[j].y; }
+            }
+        }
+    }
+}
+
 // Shared-memory carve-up of the K3 ring: chunks | full barriers | empty barriers | task counter.
 struct K3Smem {
     unsigned char *base;
@@ -275,42 +320,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
 #pragma unroll
             for (int j = 0; j < K3_SEG; ++j) { acc[0][j] = ga[j]; acc[1][j] = gb[j]; acc[2][j] = gcc[j]; }
         }
-        // ---- solve + update for K3_SEG rows x 2 columns
-        const bool pair_ok = gx + 1 < W;
-        const bool vec_out = (p.out_pitch & 1) == 0 && pair_ok;
-        float *uo = p.u_out + (size_t)gy0 * p.out_pitch + gx, *vo = p.v_out + (size_t)gy0 * p.out_pitch + gx;
-        float2 trs[K3_SEG], dets[K3_SEG];
-#pragma unroll
-        for (int j = 0; j < K3_SEG; ++j) {
-            float2 du, dv;
-            k3_solve_pair(acc[0][j], acc[1][j], acc[2][j], acc[3][j], acc[4][j], uu[j], vv[j], p.sp, du, dv, trs[j], dets[j]);
-            float2 un = __fadd2_rn(uu[j], du), vn = __fadd2_rn(vv[j], dv);
-            if (MK) {                                    // M3: no vector over an obstacle
-                if (!(mk[j] & 0xffu)) { un.x = 0.f; vn.x = 0.f; trs[j].x = 0.f; dets[j].x = 0.f; }
-                if (!(mk[j] >> 8)) { un.y = 0.f; vn.y = 0.f; trs[j].y = 0.f; dets[j].y = 0.f; }
-            }
-            if (j < nrows) {
-                if (vec_out) {
-                    *reinterpret_cast<float2 *>(uo + j * p.out_pitch) = un;
-                    *reinterpret_cast<float2 *>(vo + j * p.out_pitch) = vn;
-                } else {
-                    uo[j * p.out_pitch] = un.x; vo[j * p.out_pitch] = vn.x;
-                    if (pair_ok) { uo[j * p.out_pitch + 1] = un.y; vo[j * p.out_pitch + 1] = vn.y; }
-                }
-            }
-        }
-        if (p.valid) {                                   // last iteration of level 0 only
-            uint8_t *m = p.valid + (size_t)gy0 * W + gx;
-            float *d = p.det + (size_t)gy0 * pitch + gx;
-#pragma unroll
-            for (int j = 0; j < K3_SEG; ++j) {
-                if (j < nrows) {
-                    m[j * W] = trs[j].x > 0.f ? 1 : 0;
-                    d[j * pitch] = dets[j].x;
-                    if (pair_ok) { m[j * W + 1] = trs[j].y > 0.f ? 1 : 0; d[j * pitch + 1] = dets[j].y; }
-                }
-            }
-        }
+        k3_solve_store<MK>(p, acc, uu, vv, mk, gx, gy0, nrows);
     }
 }
 

@@ -20,6 +20,7 @@
 #include "of_k2.cuh"
 #include "of_k2s.cuh"
 #include "of_k3.cuh"
+#include "of_fused.cuh"
 
 // K2 variant of the unmasked kernels: 0 (default) = warp tiles with global gathers (of_k2.cuh), 1 (-DOF_K2_STREAMING) = the
 // task-queue form with the TMA-staged I2 window (of_k2s.cuh).  Both are kept bit-identical; profiles/r2_k2_streaming.md has the
@@ -43,6 +44,8 @@ struct LevelDesc {
     int k3_nrb, k3_ntasks;
     int k2s_nuy, k2s_nunits;                 // units of of_k2s.cuh: per strip, per level
     unsigned long long k2s_magic;            // ceil(2^40 / k2s_nuy)
+    float *u2, *v2;                          // second field buffer of a fused level (of_fused.cuh)
+    int f_tw, f_th, f_tiles_x, f_ntiles;     // fused coarse-level iteration: tile size and count, f_ntiles = 0: two-pass form
 };
 
 // Dynamic shared memory of the solve kernel: [0, 225280) data (K3 ring / K2 product buffers, A slots and I2 ring), then the K3
@@ -233,11 +236,34 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
         const LevelDesc L = a.lv[l];
         MaskDesc M = {};
         if (MK) M = a.md[l];
+        // fused coarse level (of_fused.cuh): the field alternates between (u, v) and (u2, v2); start so that the last iteration ends in (u, v)
+        const bool fused = !MK && L.f_ntiles > 0;
+        LevelDesc Lw = L;
+        if (fused && (a.iterations & 1)) { Lw.u = L.u2; Lw.v = L.v2; }
         if (l < top) {
-            upsample_phase<MK>(L, a.lv[l + 1], M.mask, cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
+            upsample_phase<MK>(Lw, a.lv[l + 1], M.mask, cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
             prof_stamp(a, pi);
             if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
             prof_stamp(a, pi);
+        }
+        if (fused) {
+            float *ui = Lw.u, *vi = Lw.v, *uo = (ui == L.u) ? L.u2 : L.u, *vo = (vi == L.v) ? L.v2 : L.v;
+            for (int it = 0; it < a.iterations; ++it) {
+                const bool last = (l == 0 && it == a.iterations - 1);
+                const FusedParams fp = {L.pyr[a.s1], L.pyr[a.s2], ui, vi, last ? a.u_out : uo, last ? a.v_out : vo, last ? a.valid : nullptr,
+                                        last ? a.det : nullptr, L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.f_tw, L.f_th, L.f_tiles_x, L.f_ntiles,
+                                        a.ww, a.sp, (l == top && it == 0) ? 1 : 0};
+                fused_iteration<R>(fp, solve_smem, cta, ncta);
+                prof_stamp(a, pi);                               // (four stamps per iteration, as in the two-pass form)
+                prof_stamp(a, pi);
+                prof_stamp(a, pi);
+                if (!last) { if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads(); }
+                prof_stamp(a, pi);
+                float *tu = ui, *tv = vi;
+                ui = uo; vi = vo; uo = tu; vo = tv;
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the tile buffers were written by generic stores; a K3 pass copies into them
+            continue;
         }
         int k2_b, k2_e, k3_b, k3_e;                              // this CTA's share of the level's tiles and tasks
         cta_range(MK ? M.k2_n : (SOLVE_K2S ? L.k2s_nunits : L.k2_ntiles), cta, ncta, k2_b, k2_e);

@@ -92,6 +92,9 @@ struct of_context {
     Level lv[OF_MAX_LEVELS];
     float *pyr[N_PYR][OF_MAX_LEVELS];
     float *u[OF_MAX_LEVELS], *v[OF_MAX_LEVELS];
+    float *u2[OF_MAX_LEVELS], *v2[OF_MAX_LEVELS];      // second field buffer of the levels iterated in fused form (of_fused.cuh)
+    int f_tw[OF_MAX_LEVELS], f_th[OF_MAX_LEVELS], f_tiles_x[OF_MAX_LEVELS], f_ntiles[OF_MAX_LEVELS];
+    bool fuse_coarse;                   // of_set_fused: coarse levels iterate inside the CTA (default on)
     float *S;
     size_t plane;
     float *det;
@@ -201,8 +204,26 @@ template <int R> K3Plan plan_k3(int W, int H, int sms)
     return p;
 }
 
+// Fused coarse-level iteration (of_fused.cuh): one tile per CTA, tile + window halo in shared memory.  Chosen when the level can be
+// cut into at most `sms` tiles that fit; among those the tiling with the fewest product pixels (tile + halo) per CTA.
+template <int R> void plan_fused(of_context *c, int l)
+{
+    typedef FusedGeom<R> G;
+    const int W = c->lv[l].W, H = c->lv[l].H;
+    long best = -1;
+    c->f_tw[l] = c->f_th[l] = c->f_tiles_x[l] = c->f_ntiles[l] = 0;
+    for (int tw = 8; tw <= 256; tw += 8)
+        for (int th = K3_SEG; th <= 256; th += K3_SEG) {
+            const int tx = (W + tw - 1) / tw, ty = (H + th - 1) / th;
+            if (tx * ty > c->sms || G::smem_bytes(tw, th) > K3_RING * K3_CHUNK_BYTES) continue;
+            const long cost = (long)G::pw(tw) * G::ph(th) * 3 + (long)tw * G::ph(th) * 2 + (long)tw * th * 5;   // products, hsum, vsum + solve
+            if (best < 0 || cost < best) { best = cost; c->f_tw[l] = tw; c->f_th[l] = th; c->f_tiles_x[l] = tx; c->f_ntiles[l] = tx * ty; }
+        }
+}
+
 template <int R> void plan_level(of_context *c, int l)
 {
+    plan_fused<R>(c, l);
     c->k2[l] = plan_k2<R>(c->lv[l].W, c->lv[l].H, c->sms);
     c->k3[l] = plan_k3<R>(c->lv[l].W, c->lv[l].H, c->sms);
     c->k2s_nuy[l] = (c->lv[l].H + K2S<R>::RU - 1) / K2S<R>::RU;
@@ -616,7 +637,8 @@ int upload_level_descs(of_context *c)
     for (int l = 0; l < c->levels; ++l)
         hl[l] = {{c->pyr[0][l], c->pyr[1][l]}, c->u[l], c->v[l], c->lv[l].W, c->lv[l].H, c->lv[l].pitch,
                  c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks,
-                 c->k2s_nuy[l], c->k2s_nunits[l], k2s_magic(c->k2s_nuy[l])};
+                 c->k2s_nuy[l], c->k2s_nunits[l], k2s_magic(c->k2s_nuy[l]), c->u2[l], c->v2[l],
+                 c->f_tw[l], c->f_th[l], c->f_tiles_x[l], (c->fuse_coarse && !c->md[l].mask) ? c->f_ntiles[l] : 0};
     CU_TRY(cudaMemcpy(c->d_lv, hl, sizeof(LevelDesc) * c->levels, cudaMemcpyHostToDevice));
     CU_TRY(cudaMemcpy(c->d_md, c->md, sizeof(MaskDesc) * c->levels, cudaMemcpyHostToDevice));
     return OF_OK;
@@ -718,7 +740,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     if (!c) { fail(OF_ERR_ALLOC, "out of host memory"); return nullptr; }
     c->W = width; c->H = height; c->levels = levels; c->R = window_radius; c->iterations = iterations;
     c->window_type = window_type; c->device = dev; c->eps_rel = 1e-3f; c->max_step = 3.0f;
-    c->use_graph = true; c->stamp = 0; c->last_launches = 0;
+    c->use_graph = true; c->stamp = 0; c->last_launches = 0; c->fuse_coarse = true;
     memcpy(c->lv, lv, sizeof lv);
     memset(&c->ww, 0, sizeof c->ww);
     for (int t = -window_radius; t <= window_radius; ++t) {
@@ -733,8 +755,12 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     for (int l = 0; l < levels && rc == OF_OK; ++l) {
         size_t bytes = sizeof(float) * (size_t)lv[l].pitch * lv[l].H;
         for (int s = 0; s < N_PYR && rc == OF_OK; ++s) rc = dev_alloc(c, (void **)&c->pyr[s][l], bytes);
-        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->u[l], 2 * bytes);      // u then v: one (x, y, {u, v}) tensor for the K2 copies
-        if (rc == OF_OK) c->v[l] = c->u[l] + (size_t)lv[l].pitch * lv[l].H;
+        if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->u[l], 4 * bytes);      // u, v, u2, v2
+        if (rc == OF_OK) {
+            c->v[l] = c->u[l] + (size_t)lv[l].pitch * lv[l].H;
+            c->u2[l] = c->v[l] + (size_t)lv[l].pitch * lv[l].H;
+            c->v2[l] = c->u2[l] + (size_t)lv[l].pitch * lv[l].H;
+        }
     }
     c->plane = (size_t)lv[0].pitch * lv[0].H;
     if (rc == OF_OK) rc = dev_alloc(c, (void **)&c->S, sizeof(float) * 5 * c->plane);
@@ -746,8 +772,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         for (int l = 0; l < levels; ++l) {
             size_t bytes = sizeof(float) * (size_t)lv[l].pitch * lv[l].H;
             for (int s = 0; s < N_PYR; ++s) cudaMemset(c->pyr[s][l], 0, bytes);
-            cudaMemset(c->u[l], 0, bytes);
-            cudaMemset(c->v[l], 0, bytes);
+            cudaMemset(c->u[l], 0, 4 * bytes);
         }
         cudaMemset(c->S, 0, sizeof(float) * 5 * c->plane);
         cudaMemset(c->det, 0, sizeof(float) * c->plane);
@@ -878,6 +903,16 @@ int of_set_persistent(of_handle h, int enable)
     h->persistent = enable != 0;
     drop_graphs(h);
     return OF_OK;
+}
+
+int of_set_fused(of_handle h, int enable)
+{
+    if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
+    h->fuse_coarse = enable != 0;
+    drop_graphs(h);
+    CU_TRY(cudaSetDevice(h->device));
+    CU_TRY(cudaDeviceSynchronize());
+    return upload_level_descs(h);
 }
 
 int of_set_hoist(of_handle h, int enable)

@@ -15,8 +15,12 @@
  *     = ordinary host memory.  Streams are cudaStream_t passed as void* (NULL = default stream).
  *   - every int-returning call returns OF_OK (0) or a negative of_status; of_last_error() gives the
  *     text of the calling thread's last failure.  No C++ exception crosses this boundary.
- *   - a handle is not thread-safe; distinct handles are independent.  There is no CPU fallback:
- *     without a usable CUDA device of_create fails.
+ *   - a handle is not thread-safe; distinct handles are independent.  All scratch belongs to the handle, so only ONE solve of a
+ *     handle is in flight at a time: a call on another stream than the previous one is ordered after it (an event wait that the
+ *     library enqueues itself); use several handles for concurrent solves.  There is no CPU fallback: without a usable CUDA
+ *     device of_create fails.
+ *   - alignment: u, v must be 16-byte aligned (the last pass stores vectors), I1, I2 to their element size; a pointer that is
+ *     not is rejected with OF_ERR_INVALID_ARG.
  *   - results are bit-reproducible for the same inputs (no atomics in any sum).
  */
 #ifndef OPTFLOW_H_
@@ -56,7 +60,9 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
 
 /* Solve one pair.  I1, I2: device pointers, fp32, dense H x W, read-only.  u, v: device pointers,
  * fp32, dense H x W, write-only (the initial guess is always zero).  Everything is
- * enqueued on `stream`; the call never synchronises or allocates.  Steps enqueued (DESIGN.md
+ * enqueued on `stream`; the call never synchronises and allocates no device memory (the launch sequence is replayed as a CUDA
+ * graph: the first call with a new set of pointers captures it, later calls replay it; beyond 64 cached sets the least recently
+ * used graph is re-parameterised in place).  Steps enqueued (DESIGN.md
  * "Kernels"): pyramid build of both images, zero field at the coarsest level, then per level
  * coarse-to-fine: x2 flow upsampling, and `iterations` x { warp + gradients + five products +
  * horizontal window sum ; vertical window sum + damped 2x2 solve + in-place (u,v) update }. */
@@ -209,6 +215,12 @@ int of_stream_submit(of_handle h);
  * of_stream_open), valid until the second-next of_stream_result call.  *pair_index (optional)
  * receives its 0-based index.  OF_ERR_STATE if nothing is pending. */
 int of_stream_result(of_handle h, const float **u, const float **v, int *pair_index);
+
+/* Validity bytes (H x W, 1 = tr(G) > 0, D14) of the field the last of_stream_result returned: every slot of the result ring has
+ * its own plane, written by the last pass of that pair's solve and copied with the field, so the mask belongs to the returned
+ * field even while the next pair is being solved (eq. 3 counts "available vectors").  Host pointer if the pipeline
+ * was opened with result_on_host, else device pointer; valid as long as the field's pointers. */
+int of_stream_result_validity(of_handle h, const uint8_t **valid);
 /* Drain and release the pipeline's buffers. */
 int of_stream_close(of_handle h);
 

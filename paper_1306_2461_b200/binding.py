@@ -16,6 +16,7 @@ OF_WINDOW_BOX, OF_WINDOW_GAUSSIAN = 0, 1
 OF_DTYPE_F32, OF_DTYPE_U8, OF_DTYPE_U16 = 0, 1, 2
 OF_STREAM_CONSECUTIVE, OF_STREAM_PAIRS = 0, 1
 OF_OK = 0
+OF_ERR_INVALID_ARG, OF_ERR_ALLOC, OF_ERR_CUDA, OF_ERR_STATE = -1, -2, -3, -4
 
 _c = ctypes
 _vp, _i = _c.c_void_p, _c.c_int
@@ -35,6 +36,7 @@ SIGNATURES = {
     "of_set_persistent": (_i, [_vp, _i]),
     "of_set_hoist": (_i, [_vp, _i]),
     "of_set_fused": (_i, [_vp, _i]),
+    "of_stream_result_validity": (_i, [_vp, ctypes.POINTER(ctypes.c_void_p)]),
     "of_solve_timeline": (_i, [_vp, _i, _i, _vp, _i]),
     "of_get_validity": (_i, [_vp, _vp, _vp]),
     "of_level_size": (_i, [_vp, _i, _c.POINTER(_i), _c.POINTER(_i)]),
@@ -137,6 +139,8 @@ class OpticalFlow:
             u = torch.empty((self.height, self.width), dtype=torch.float32, device=I1.device)
         if v is None:
             v = torch.empty((self.height, self.width), dtype=torch.float32, device=I1.device)
+        for f in (u, v):
+            assert f.is_cuda and f.is_contiguous() and f.dtype == torch.float32 and tuple(f.shape) == (self.height, self.width)
         if I1.dtype == torch.float32:
             fn = lib().of_compute
         elif I1.dtype == torch.uint8:
@@ -265,8 +269,41 @@ class OpticalFlow:
         v = np.frombuffer((ctypes.c_float * n).from_address(pv.value), dtype=np.float32).reshape(self.height, self.width)
         return idx.value, u, v
 
+    def stream_result_validity(self):
+        """Validity bytes of the field the last stream_result returned (host mode: NumPy view; device mode: raw pointer)."""
+        import numpy as np
+        pm = _vp()
+        _check(lib().of_stream_result_validity(self._h, ctypes.byref(pm)))
+        if not self._s_host:
+            return pm.value
+        n = self.width * self.height
+        return np.frombuffer((ctypes.c_uint8 * n).from_address(pm.value), dtype=np.uint8).reshape(self.height, self.width)
+
     def stream_close(self):
         _check(lib().of_stream_close(self._h))
+
+
+def device_to_numpy(ptr: int, count: int, dtype):
+    """Copy `count` elements from a raw device pointer (as the pipeline hands out in device-result mode) into a NumPy array.
+    Synchronous cudaMemcpy through the CUDA runtime that torch has loaded."""
+    import numpy as np
+    import torch  # noqa: F401  (loads libcudart)
+    rt = None
+    for name in ("libcudart.so.12", "libcudart.so"):
+        try:
+            rt = ctypes.CDLL(name)
+            break
+        except OSError:
+            continue
+    if rt is None:
+        raise OptflowError("libcudart not found")
+    out = np.empty(count, dtype=dtype)
+    rt.cudaMemcpy.restype = ctypes.c_int
+    rt.cudaMemcpy.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int]
+    err = rt.cudaMemcpy(out.ctypes.data, ptr, out.nbytes, 2)          # cudaMemcpyDeviceToHost
+    if err != 0:
+        raise OptflowError("cudaMemcpy failed: error %d" % err)
+    return out
 
 
 def pyramid_down(src, stream=None):

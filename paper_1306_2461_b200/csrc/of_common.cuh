@@ -5,6 +5,14 @@
 
 #define OFK_MAX_R 16
 
+// Profiling switches of the kernels (phases switched off one by one, profiles/r1_launch_overhead.md) exist in -DOF_PROFILE builds
+// only: in the shipped build OF_DBG() is a compile-time 0 and the switches cost neither instructions nor registers.
+#ifdef OF_PROFILE
+#define OF_DBG(flags, bit) ((flags) & (bit))
+#else
+#define OF_DBG(flags, bit) 0
+#endif
+
 struct WinWeights { float w[2 * OFK_MAX_R + 1]; };   // w[t + R], t = -R..R; passed by value (param bank)
 
 __device__ __forceinline__ int clampi(int i, int lo, int hi) { return max(lo, min(i, hi)); }

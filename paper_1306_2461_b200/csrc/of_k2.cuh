@@ -45,7 +45,7 @@ struct K2Params {
     WinWeights ww;
     int zero_uv;                                   // 1 = the field is identically zero (first iteration at the coarsest level,
                                                    // PAPER.md:61 "initial guess of zero displacement"): u, v are not read
-    int dbg;                                       // profiling switches (0 in production): 1 = no product phase, 2 = no sum phase, 32 = no plane stores
+    int dbg;                                       // -DOF_PROFILE builds only: 1 = no product phase, 2 = no sum phase, 32 = no plane stores
     const uint8_t *mask;                           // obstacle mask of the level (pitch = `pitch`) or NULL (M2: zero weight)
     const int *list;                               // compacted tile list (then ntiles = its length) or NULL
     int f_first;                                   // first plane this pass forms: 0 = all five; 3 = IxIt, IyIt only (of_set_hoist:
@@ -231,7 +231,8 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
         // round's gathers wait for one L2 round trip (I1 / I2) instead of two (u, v, then I2).  Measured (profiles/r1_experiments.md):
         // level-0 K2 pass 16.0 -> 15.1 us at 1280x1024, 57.2 -> 50.1 us at 2048x2048; one-round tiles of the coarse levels lose
         // 0.4 us with it (unrolled guards), so they keep the rolled loop below.
-        constexpr int MAXR = 6;
+        constexpr int MAXR = 6;                            // product rounds of the widest tile: (nseg <= 32: 128 + RL column pairs) / 32
+        static_assert(128 + 4 * G::RL <= 32 * MAXR, "MAXR too small for the widest warp tile");
         float2 pu0[MAXR], pu1[MAXR], pv0[MAXR], pv1[MAXR];
 #pragma unroll
         for (int r = 0; r < MAXR; ++r) {
@@ -252,7 +253,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
 #pragma unroll
         for (int r = 0; r < MAXR; ++r) {
             const int k = lane + 32 * r;
-            if (32 * r >= ntasks || k >= ntasks || (p.dbg & 1)) continue;
+            if (32 * r >= ntasks || k >= ntasks || OF_DBG(p.dbg, 1)) continue;
             int rp = 0, cp = k;
             while (cp >= half) { cp -= half; ++rp; }
             const int x = xs + 2 * cp, y = y0 + 2 * rp;
@@ -274,7 +275,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
         }
         } else
 #pragma unroll 1
-        for (int k = lane; k < ntasks && !(p.dbg & 1); k += 32) {
+        for (int k = lane; k < ntasks && !OF_DBG(p.dbg, 1); k += 32) {
             int rp = 0, cp = k;
             while (cp >= half) { cp -= half; ++rp; }
             const int x = xs + 2 * cp, y = y0 + 2 * rp;
@@ -296,7 +297,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
         __syncwarp();
 
         // ---------------- phase 2: horizontal window sum, 8 outputs x 2 rows per lane
-        if (h_f0 < nf_par && !(p.dbg & 2)) {
+        if (h_f0 < nf_par && !OF_DBG(p.dbg, 2)) {
             const int gx = x0 + 8 * h_seg, gy = y0 + 2 * h_rp;
             const char *src = sm + h_rp * BB + h_seg * 80;
 #pragma unroll 1
@@ -324,7 +325,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
                     for (int j = 0; j < 8; ++j)
                         if (i - j - G::OFF >= 0 && i - j - G::OFF <= 2 * R) acc[j] = fma2s(p.ww.w[i - j - G::OFF], in[i], acc[j]);
 #endif
-                if (gx < pitch && (!(p.dbg & 32) || acc[0].x == 12345.678f)) {
+                if (gx < pitch && !OF_DBG(p.dbg, 32)) {
                     float *d0 = p.S + f * p.plane + (size_t)gy * pitch + gx;
                     if (gy < H) {
                         *reinterpret_cast<float4 *>(d0) = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);

@@ -53,7 +53,7 @@ struct K3Params {
     WinWeights ww;
     SolveParams sp;
     int zero_uv;                     // 1 = the incoming field is identically zero and is not read (see of_k2.cuh)
-    int dbg;                         // profiling switches (0 in production): 1 = no TMA/no waits, 2 = no window sum, 4 = no solve
+    int dbg;                         // -DOF_PROFILE builds only: 1 = no TMA/no waits, 2 = no window sum, 4 = no solve
     MaskDesc md;                     // obstacle mask and compacted task lists of the level (all zero: none)
     float *G;                        // of_set_hoist: three planes (stride `gplane`, pitch `pitch`) holding the window sums a, b, c
     size_t gplane;                   //   of IxIx, IxIy, IyIy of the level (written by an HM = 1 pass, read by HM = 2 passes)
@@ -193,7 +193,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         // One lane needs ~105 cycles per bulk tensor copy (expect_tx + issue; measured, profiles/r2_tma_issue.md), so a single
         // lane delivered the ~40 chunks of a level-0 pass only after ~6700 cycles; 32 lanes have them in flight after ~2300.
         // Consumers wait on the full barrier of each chunk, so the order of issue does not matter.
-        if (!(p.dbg & 1)) {
+        if (!OF_DBG(p.dbg, 1)) {
             // one run = `ntask` consecutive tasks of strip s from row block rb0; its chunks start at ring chunk gbase
             auto produce_run = [&](int s, int rb0, int ntask, int gbase) {
                 const int total = ntask + NC - 1;
@@ -288,10 +288,10 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
         for (int f = 0; f < 5; ++f)
 #pragma unroll
             for (int j = 0; j < K3_SEG; ++j) acc[f][j] = make_float2(0.f, 0.f);
-        if (!(p.dbg & 2))
+        if (!OF_DBG(p.dbg, 2))
 #pragma unroll
         for (int r = 0; r < G::NIN; ++r) {
-            if ((r % K3_SEG) == 0 && !(p.dbg & 1)) mbar_wait(fb[r / K3_SEG], fpar[r / K3_SEG]);   // chunk by chunk, as the TMA delivers them
+            if ((r % K3_SEG) == 0 && !OF_DBG(p.dbg, 1)) mbar_wait(fb[r / K3_SEG], fpar[r / K3_SEG]);   // chunk by chunk, as the TMA delivers them
 #pragma unroll
             for (int f = F0; f < 5; ++f) {
                 const float2 val = *reinterpret_cast<const float2 *>(cb[r / K3_SEG] + (f - F0) * (K3_SEG * 256) + (r % K3_SEG) * 256);
@@ -301,11 +301,11 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             }
         }
         __syncwarp();
-        if (lane == 0 && !(p.dbg & 1)) {
+        if (lane == 0 && !OF_DBG(p.dbg, 1)) {
 #pragma unroll
             for (int k = 0; k < NC; ++k) mbar_arrive(eb[k], 1);
         }
-        if (!active || (p.dbg & 4)) continue;
+        if (!active || OF_DBG(p.dbg, 4)) continue;
         if (HM == 1) {                                   // keep a, b, c for the later iterations of the level
             float *gp = p.G + (size_t)gy0 * pitch + gx;
 #pragma unroll

@@ -243,7 +243,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
         if (l < top) {
             upsample_phase<MK>(Lw, a.lv[l + 1], M.mask, cta * blockDim.x + threadIdx.x, ncta * blockDim.x);
             prof_stamp(a, pi);
-            if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
+            if (!OF_DBG(a.dbg, 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
             prof_stamp(a, pi);
         }
         if (fused) {
@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
                 prof_stamp(a, pi);                               // (four stamps per iteration, as in the two-pass form)
                 prof_stamp(a, pi);
                 prof_stamp(a, pi);
-                if (!last) { if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads(); }
+                if (!last) { if (!OF_DBG(a.dbg, 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads(); }
                 prof_stamp(a, pi);
                 float *tu = ui, *tv = vi;
                 ui = uo; vi = vo; uo = tu; vo = tv;
@@ -289,7 +289,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             prof_stamp(a, pi);
-            if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
+            if (!OF_DBG(a.dbg, 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads();
             prof_stamp(a, pi);
             // ---- K3 pass: vertical sums + solve + update
             const bool last = (l == 0 && it == a.iterations - 1);
@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             __syncthreads();
             if (threadIdx.x == 0) { sm.counter[0] = 0; sm.counter[1] = 0; }
             prof_stamp(a, pi);
-            if (!last) { if (!(a.dbg & 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads(); }
+            if (!last) { if (!OF_DBG(a.dbg, 8)) grid_barrier(a.gbar, ncta, nbar); else __syncthreads(); }
             prof_stamp(a, pi);
         }
     }

@@ -58,6 +58,7 @@ struct Job {
     int cvtA, cvtB;            // pyramid slots to (re)build, -1 = none
     int s1, s2;                // pyramid slots used as I1 / I2
     float *u_out, *v_out;      // level-0 result, dense
+    uint8_t *valid_out;        // validity bytes of the result (the handle's own plane, or a slot of the streaming result ring)
     bool operator==(const Job &o) const { return memcmp(this, &o, sizeof(Job)) == 0; }
 };
 
@@ -74,12 +75,13 @@ struct Pipeline {
     cudaStream_t s_copy = nullptr, s_comp = nullptr, s_down = nullptr;
     void *pin[N_PIN] = {nullptr, nullptr};
     void *raw[N_PIN] = {nullptr, nullptr};
-    float *res_dev[N_RES] = {};
+    float *res_dev[N_RES] = {};            // per slot: u, v (2 x field_bytes), then the validity bytes (W*H)
     float *res_host[N_RES] = {};
     cudaEvent_t h2d_done[N_PIN] = {}, cvt_done[N_PIN] = {}, solve_done[N_RES] = {}, d2h_done[N_RES] = {};
     bool cvt_rec[N_PIN] = {}, d2h_rec[N_RES] = {};
     long long acquired = 0, submitted = 0, produced = 0, collected = 0;
     int cur_slot = -1;
+    const uint8_t *last_valid = nullptr;   // validity bytes of the field of_stream_result returned last
 };
 
 }  // namespace
@@ -128,6 +130,10 @@ struct of_context {
     int zero_n;
     std::vector<void *> mask_allocs;
     Pipeline pipe;
+    cudaEvent_t last_done;             // recorded after every submit (one solve in flight per handle)
+    cudaStream_t last_stream;
+    bool have_last;
+    float *bench_out;                  // of_run_solve: a dense u, v pair of its own for the discarded result
 };
 
 namespace {
@@ -155,8 +161,10 @@ template <int R> K2Plan plan_k2(int W, int H, int sms, double active = 1.0)   //
     typedef K2Geom<R> G;
     K2Plan best = {};
     double best_cost = 1e30;
-    int f_nseg = 0, f_nrp = 0;
+    int f_nseg = 0, f_nrp = 0;                     // (-DOF_PROFILE builds: tile shape forced through the environment, for sweeps)
+#ifdef OF_PROFILE
     if (const char *e = getenv("OF_K2_GEOM")) sscanf(e, "%d,%d", &f_nseg, &f_nrp);
+#endif
     const int segs = (W + 7) / 8;
     for (int nrp = 1; nrp <= 4; nrp *= 2) {
         const int nsegmax = 32 / nrp, tx_min = (segs + nsegmax - 1) / nsegmax;
@@ -249,24 +257,24 @@ void launch_k2(const of_context *c, int l, const float *I1, const float *I2, boo
 }
 
 template <int R>
-void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st)
+void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st, uint8_t *valid_out = nullptr)
 {
     const Level &L = c->lv[l];
     const K3Plan &P = c->k3[l];
-    K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? c->valid : nullptr, last ? c->det : nullptr,
+    K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? (valid_out ? valid_out : c->valid) : nullptr, last ? c->det : nullptr,
                   L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg, c->md[l], nullptr, 0};
     if (c->md[l].mask) of_launch_k3_masked(R, c->tmS[l], p, P.grid, 32 * (P.warps + 1), P.smem, st);
     else k3_vsum_solve<R, false><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
 template <int R>
-cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int s2, float *u_out, float *v_out, cudaStream_t st)
+cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int s2, float *u_out, float *v_out, cudaStream_t st, uint8_t *valid_out = nullptr)
 {
     static_assert(SOLVE_MAX_LEVELS == OF_MAX_LEVELS, "level limits out of sync");
     SolveArgs a;
     memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
     a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
-    a.valid = c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
+    a.valid = valid_out ? valid_out : c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
     a.md = c->d_md; a.G = c->G; a.k2maps = c->d_k2maps;
     const bool ho = c->hoist && c->G != nullptr;
     if (ho) memcpy(a.tm2, c->tmS2, sizeof(CUtensorMap) * c->levels);
@@ -343,9 +351,9 @@ void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool z
 {
     DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, zero_uv, st));
 }
-void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st)
+void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st, uint8_t *valid_out = nullptr)
 {
-    DISPATCH_R(c->R, launch_k3<R>(c, l, u_out, v_out, out_pitch, last, zero_uv, st));
+    DISPATCH_R(c->R, launch_k3<R>(c, l, u_out, v_out, out_pitch, last, zero_uv, st, valid_out));
 }
 
 void run_convert(const of_context *c, int dtype, const void *a, const void *b, float *da, float *db, cudaStream_t st)
@@ -441,13 +449,13 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
     const int top = c->levels - 1;     // (no memset of the coarsest field: its first iteration takes u = v = 0 without reading it)
     if (c->persistent) {
         cudaError_t e = cudaSuccess;
-        DISPATCH_R(c->R, e = launch_solve<R>(c, nullptr, j.s1, j.s2, j.u_out, j.v_out, st));
+        DISPATCH_R(c->R, e = launch_solve<R>(c, nullptr, j.s1, j.s2, j.u_out, j.v_out, st, j.valid_out));
         if (e != cudaSuccess && c->launch_err.empty()) c->launch_err = std::string("solve (persistent): ") + cudaGetErrorString(e);
         note_launch(c, "solve (persistent)", 0);
         return n + 1;
     }
     if (c->zero_n > 0) {               // mask set: outputs of the level-0 tasks no K3 pass visits (M3)
-        k_mask_zero<<<c->sms, 256, 0, st>>>(c->d_zero, c->zero_n, c->k3[0].nrb, c->W, c->H, c->lv[0].pitch, j.u_out, j.v_out, c->W, c->valid, c->det);
+        k_mask_zero<<<c->sms, 256, 0, st>>>(c->d_zero, c->zero_n, c->k3[0].nrb, c->W, c->H, c->lv[0].pitch, j.u_out, j.v_out, c->W, j.valid_out ? j.valid_out : c->valid, c->det);
         note_launch(c, "mask zero-fill", 0);
         ++n;
     }
@@ -458,7 +466,7 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
             run_k2(c, l, c->pyr[j.s1][l], c->pyr[j.s2][l], zero_uv, st);
             note_launch(c, "products+hsum", l);
             const bool last = (l == 0 && it == c->iterations - 1);
-            if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, zero_uv, st);
+            if (last) run_k3(c, l, j.u_out, j.v_out, c->W, true, zero_uv, st, j.valid_out);
             else run_k3(c, l, c->u[l], c->v[l], c->lv[l].pitch, false, zero_uv, st);
             note_launch(c, "vsum+solve", l);
             n += 2;
@@ -467,9 +475,25 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
     return n;
 }
 
+int submit_job_inner(of_context *c, const Job &j, cudaStream_t st);
+
+// All scratch (pyramids, fields, planes, the grid-barrier word) belongs to the handle, so only one solve of a handle may be in flight:
+// a submit on another stream than the previous one is ordered after it with an event.
 int submit_job(of_context *c, const Job &j, cudaStream_t st)
 {
     CU_TRY(cudaSetDevice(c->device));
+    if (c->have_last && st != c->last_stream) CU_TRY(cudaStreamWaitEvent(st, c->last_done, 0));
+    int rc = submit_job_inner(c, j, st);
+    if (rc == OF_OK) {
+        CU_TRY(cudaEventRecord(c->last_done, st));
+        c->last_stream = st;
+        c->have_last = true;
+    }
+    return rc;
+}
+
+int submit_job_inner(of_context *c, const Job &j, cudaStream_t st)
+{
     if (!c->use_graph || st == nullptr) {
         c->last_launches = enqueue_job(c, j, st);
         cudaError_t e = cudaGetLastError();
@@ -494,17 +518,28 @@ int submit_job(of_context *c, const Job &j, cudaStream_t st)
         return fail(OF_ERR_CUDA, "graph capture failed: %s / %s; first failing launch: %s", cudaGetErrorString(e1), cudaGetErrorString(e2),
                     c->launch_err.c_str());
     }
+    if (c->graphs.size() >= 64) {
+        // cache full (a caller that rotates more than 64 pointer sets): re-use the least recently used executable graph by
+        // patching the kernel parameters of its nodes in place (cudaGraphExecUpdate: same topology, no instantiation)
+        size_t old = 0;
+        for (size_t i = 1; i < c->graphs.size(); ++i)
+            if (c->graphs[i].stamp < c->graphs[old].stamp) old = i;
+        cudaGraphExecUpdateResultInfo info;
+        if (cudaGraphExecUpdate(c->graphs[old].exec, graph, &info) == cudaSuccess) {
+            cudaGraphDestroy(graph);
+            c->graphs[old].job = j; c->graphs[old].stamp = c->stamp; c->graphs[old].launches = n;
+            CU_TRY(cudaGraphLaunch(c->graphs[old].exec, st));
+            c->last_launches = n;
+            return OF_OK;
+        }
+        (void)cudaGetLastError();
+        cudaGraphExecDestroy(c->graphs[old].exec);
+        c->graphs.erase(c->graphs.begin() + old);
+    }
     cudaGraphExec_t exec = nullptr;
     cudaError_t e3 = cudaGraphInstantiate(&exec, graph, 0);
     cudaGraphDestroy(graph);
     if (e3 != cudaSuccess) return fail(OF_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e3));
-    if (c->graphs.size() >= 64) {
-        size_t old = 0;
-        for (size_t i = 1; i < c->graphs.size(); ++i)
-            if (c->graphs[i].stamp < c->graphs[old].stamp) old = i;
-        cudaGraphExecDestroy(c->graphs[old].exec);
-        c->graphs.erase(c->graphs.begin() + old);
-    }
     c->graphs.push_back({j, exec, c->stamp, n});
     CU_TRY(cudaGraphLaunch(exec, st));
     c->last_launches = n;
@@ -625,8 +660,10 @@ int build_mask(of_context *c, const uint8_t *mask, int row_stride)
             }
         M.k2_n = (int)tiles.size();
         if ((rc = upload(tiles.data(), tiles.size() * sizeof(int), (void **)&M.k2_list)) != OF_OK) return rc;
+#ifdef OF_PROFILE
         if (getenv("OF_DEBUG"))
             fprintf(stderr, "[optflow] mask level %d: K2 tiles %d of %d, K3 tasks %d of %d (%zu runs)\n", l, M.k2_n, P2.ntiles, M.k3_n, P3.ntasks, runs.size());
+#endif
     }
     return OF_OK;
 }
@@ -663,6 +700,11 @@ int compute_any(of_handle h, int dtype, const void *I1, const void *I2, float *u
     if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
     if (!I1 || !I2 || !u || !v) return fail(OF_ERR_INVALID_ARG, "null image or field pointer");
     if (h->pipe.open) return fail(OF_ERR_STATE, "handle is in streaming mode; call of_stream_close first");
+    if ((reinterpret_cast<uintptr_t>(u) | reinterpret_cast<uintptr_t>(v)) & 15)
+        return fail(OF_ERR_INVALID_ARG, "u and v must be 16-byte aligned (the last pass stores float2 / float4)");
+    const size_t es = dtype == OF_DTYPE_U8 ? 1 : (dtype == OF_DTYPE_U16 ? 2 : 4);
+    if ((reinterpret_cast<uintptr_t>(I1) | reinterpret_cast<uintptr_t>(I2)) & (es - 1))
+        return fail(OF_ERR_INVALID_ARG, "I1 and I2 must be aligned to their element size");
     Job j;
     memset(&j, 0, sizeof j);
     j.dtype = dtype; j.rawA = I1; j.rawB = I2; j.cvtA = 0; j.cvtB = 1; j.s1 = 0; j.s2 = 1; j.u_out = u; j.v_out = v;
@@ -741,6 +783,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     c->W = width; c->H = height; c->levels = levels; c->R = window_radius; c->iterations = iterations;
     c->window_type = window_type; c->device = dev; c->eps_rel = 1e-3f; c->max_step = 3.0f;
     c->use_graph = true; c->stamp = 0; c->last_launches = 0; c->fuse_coarse = true;
+    c->last_done = nullptr; c->last_stream = nullptr; c->have_last = false; c->bench_out = nullptr;
     memcpy(c->lv, lv, sizeof lv);
     memset(&c->ww, 0, sizeof c->ww);
     for (int t = -window_radius; t <= window_radius; ++t) {
@@ -779,6 +822,8 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
         cudaMemset(c->valid, 0, (size_t)width * height);
         if (cudaDeviceSynchronize() != cudaSuccess) rc = fail(OF_ERR_CUDA, "memset failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
+    if (rc == OF_OK && cudaEventCreateWithFlags(&c->last_done, cudaEventDisableTiming) != cudaSuccess)
+        rc = fail(OF_ERR_CUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc == OF_OK) { DISPATCH_R(window_radius, rc = setup_attrs<R>()); }
     if (rc == OF_OK) {
         cudaError_t e = of_setup_attrs_hoisted(window_radius, SMEM_MAX);
@@ -787,7 +832,10 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     }
     if (rc == OF_OK) {
         c->sms = prop.multiProcessorCount;
+        c->dbg = 0;
+#ifdef OF_PROFILE
         c->dbg = getenv("OF_KERNEL_DEBUG") ? atoi(getenv("OF_KERNEL_DEBUG")) : 0;
+#endif
         for (int l = 0; l < levels; ++l) { DISPATCH_R(window_radius, plan_level<R>(c, l)); }
         rc = dev_alloc(c, (void **)&c->d_k2maps, sizeof(K2SMaps) * levels);
         if (rc == OF_OK) rc = encode_tensor_maps(c);
@@ -804,13 +852,15 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
             if (cudaDeviceSynchronize() != cudaSuccess) rc = fail(OF_ERR_CUDA, "descriptor upload failed: %s", cudaGetErrorString(cudaGetLastError()));
             int coop = 0;
             cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-            c->persistent = coop != 0 && !(getenv("OF_PERSISTENT") && atoi(getenv("OF_PERSISTENT")) == 0);
+            c->persistent = coop != 0;
         }
+#ifdef OF_PROFILE
         if (getenv("OF_DEBUG"))
             for (int l = 0; l < levels; ++l)
                 fprintf(stderr, "[optflow] level %d %dx%d pitch %d | K2 nseg %d nrp %d tiles %d grid %d warps %d smem %d | K3 tasks %d grid %d warps %d smem %d\n",
                         l, lv[l].W, lv[l].H, lv[l].pitch, c->k2[l].nseg, c->k2[l].nrp, c->k2[l].ntiles, c->k2[l].grid, c->k2[l].warps,
                         c->k2[l].smem, c->k3[l].ntasks, c->k3[l].grid, c->k3[l].warps, c->k3[l].smem);
+#endif
     }
     if (rc != OF_OK) { std::string keep = g_err; of_destroy(c); g_err = keep; return nullptr; }
     return c;
@@ -823,6 +873,7 @@ void of_destroy(of_handle h)
     if (h->pipe.open) pipe_release(h);
     cudaDeviceSynchronize();
     drop_graphs(h);
+    if (h->last_done) cudaEventDestroy(h->last_done);
     for (void *p : h->allocs) cudaFree(p);
     for (void *p : h->mask_allocs) cudaFree(p);
     delete h;
@@ -1004,10 +1055,13 @@ int of_run_solve(of_handle h, int repeat, void *stream)
     if (!h->persistent) return fail(OF_ERR_STATE, "persistent mode is off");
     CU_TRY(cudaSetDevice(h->device));
     cudaStream_t st = (cudaStream_t)stream;
+    if (!h->bench_out) {                                  // the discarded result gets a dense u, v pair of its own (first call only)
+        int rc = dev_alloc(h, (void **)&h->bench_out, sizeof(float) * 2 * (size_t)h->W * h->H);
+        if (rc != OF_OK) return rc;
+    }
     for (int i = 0; i < repeat; ++i) {
         cudaError_t e = cudaSuccess;
-        // the level-0 result goes to the handle's own scratch (first two planes of S are free after the solve)
-        DISPATCH_R(h->R, e = launch_solve<R>(h, nullptr, 0, 1, h->S + 3 * h->plane, h->S + 4 * h->plane, st));
+        DISPATCH_R(h->R, e = launch_solve<R>(h, nullptr, 0, 1, h->bench_out, h->bench_out + (size_t)h->W * h->H, st));
         if (e != cudaSuccess) return fail(OF_ERR_CUDA, "solve launch failed: %s", cudaGetErrorString(e));
     }
     return OF_OK;
@@ -1094,8 +1148,8 @@ int of_stream_open(of_handle h, int dtype, int mode, int result_on_host)
         ok(cudaEventCreateWithFlags(&p.cvt_done[i], cudaEventDisableTiming));
     }
     for (int i = 0; i < N_RES; ++i) {
-        ok(cudaMalloc((void **)&p.res_dev[i], 2 * p.field_bytes));
-        if (p.host_result) ok(cudaHostAlloc((void **)&p.res_host[i], 2 * p.field_bytes, cudaHostAllocDefault));
+        ok(cudaMalloc((void **)&p.res_dev[i], 2 * p.field_bytes + (size_t)h->W * h->H));
+        if (p.host_result) ok(cudaHostAlloc((void **)&p.res_host[i], 2 * p.field_bytes + (size_t)h->W * h->H, cudaHostAllocDefault));
         ok(cudaEventCreateWithFlags(&p.solve_done[i], cudaEventDisableTiming));
         ok(cudaEventCreateWithFlags(&p.d2h_done[i], cudaEventDisableTiming));
     }
@@ -1152,6 +1206,7 @@ int of_stream_submit(of_handle h)
         if (p.d2h_rec[r]) CU_TRY(cudaStreamWaitEvent(p.s_comp, p.d2h_done[r], 0));
         j.u_out = p.res_dev[r];
         j.v_out = p.res_dev[r] + (size_t)h->W * h->H;
+        j.valid_out = reinterpret_cast<uint8_t *>(p.res_dev[r] + 2 * (size_t)h->W * h->H);
         int rc = submit_job(h, j, p.s_comp);
         if (rc != OF_OK) return rc;
         CU_TRY(cudaEventRecord(p.cvt_done[s], p.s_comp));   // (recorded after the solve: conservative)
@@ -1159,7 +1214,7 @@ int of_stream_submit(of_handle h)
         CU_TRY(cudaEventRecord(p.solve_done[r], p.s_comp));
         if (p.host_result) {
             CU_TRY(cudaStreamWaitEvent(p.s_down, p.solve_done[r], 0));
-            CU_TRY(cudaMemcpyAsync(p.res_host[r], p.res_dev[r], 2 * p.field_bytes, cudaMemcpyDeviceToHost, p.s_down));
+            CU_TRY(cudaMemcpyAsync(p.res_host[r], p.res_dev[r], 2 * p.field_bytes + (size_t)h->W * h->H, cudaMemcpyDeviceToHost, p.s_down));
             CU_TRY(cudaEventRecord(p.d2h_done[r], p.s_down));
             p.d2h_rec[r] = true;
         }
@@ -1190,7 +1245,17 @@ int of_stream_result(of_handle h, const float **u, const float **v, int *pair_in
     if (u) *u = base;
     if (v) *v = base + (size_t)h->W * h->H;
     if (pair_index) *pair_index = (int)p.collected;
+    p.last_valid = reinterpret_cast<const uint8_t *>(base + 2 * (size_t)h->W * h->H);
     ++p.collected;
+    return OF_OK;
+}
+
+int of_stream_result_validity(of_handle h, const uint8_t **valid)
+{
+    if (!h || !h->pipe.open) return fail(OF_ERR_STATE, "pipeline not open");
+    if (!valid) return fail(OF_ERR_INVALID_ARG, "null argument");
+    if (!h->pipe.last_valid) return fail(OF_ERR_STATE, "no field has been collected yet");
+    *valid = h->pipe.last_valid;
     return OF_OK;
 }
 

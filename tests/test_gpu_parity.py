@@ -189,23 +189,59 @@ def test_upsample_step_matches_oracle(torch, B, oracle):
 
 
 def test_intermediates_per_level(torch, B, oracle):
-    """Pyramid levels, the per-level fields and det against the oracle's intermediates."""
+    """Pyramid levels, the per-level fields (rule D23 applied at every level: element-wise on the pixels whose determinant exceeds
+    1e-3 of the level's maximum) and det against the oracle's intermediates."""
     c = syn.config3(352, 288)
     ref = oracle.solve(c.I1, c.I2, 3, 6, 3, GAUSS, return_levels=True)
     with B.OpticalFlow(352, 288, 3, 6, 3, GAUSS) as of:
         u, v = of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda())
         torch.cuda.synchronize()
-        P = c.I1.astype(np.float64)
+        P1, P2 = c.I1.astype(np.float64), c.I2.astype(np.float64)
         for l in range(3):
             g = of.debug_plane(l, 0).cpu().numpy()
-            assert np.max(np.abs(g - P)) < 1e-4, l
+            assert np.max(np.abs(g - P1)) < 1e-4, l
             if l >= 1:
-                gu = of.debug_plane(l, 2).cpu().numpy()
-                S = np.ones_like(gu, dtype=bool)
-                assert np.sqrt(np.mean((gu - ref["level_u"][l]) ** 2)) < 1e-3, l
-            P = oracle.downsample(P)
+                gu = of.debug_plane(l, 2).cpu().numpy().astype(np.float64)
+                gv = of.debug_plane(l, 3).cpu().numpy().astype(np.float64)
+                det_l = oracle.iteration(P1, P2, np.zeros_like(P1), np.zeros_like(P1), 6, GAUSS)[4]     # iteration independent (D9)
+                S = det_l > 1e-3 * det_l.max()
+                du, dv = (gu - ref["level_u"][l])[S], (gv - ref["level_v"][l])[S]
+                assert S.mean() > 0.5 and max(np.abs(du).max(), np.abs(dv).max()) <= 1e-3, (l, np.abs(du).max(), np.abs(dv).max())
+                assert np.sqrt(np.mean(du * du + dv * dv)) <= 1e-4, l
+            P1, P2 = oracle.downsample(P1), oracle.downsample(P2)
         det = of.debug_plane(0, 9).cpu().numpy()
         assert np.max(np.abs(det - ref["det"])) <= 1e-4 * ref["det"].max()
+
+
+@pytest.mark.parametrize("W,H,R,wt", [(192, 160, 8, BOX), (203, 131, 12, GAUSS)])
+def test_k2_planes_and_window_sums_elementwise(torch, B, oracle, W, H, R, wt):
+    """K2 on its own: the five horizontally summed product planes (debug planes 4..8) after one stand-alone K2 pass from a non-zero
+    field, element by element against the oracle's warp / gradients / products summed along x; and those planes summed along y
+    against the oracle's window sums a, b, c, p, q (sums5).  Zero extension outside the image (D12) in both directions."""
+    from scipy.ndimage import correlate1d
+    c = syn.config1(W, H)
+    I1, I2 = c.I1.astype(np.float64), c.I2.astype(np.float64)
+    with B.OpticalFlow(W, H, 1, R, 2, wt) as of:
+        of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda())
+        torch.cuda.synchronize()
+        u0 = of.debug_plane(0, 2).cpu().numpy().astype(np.float64)
+        v0 = of.debug_plane(0, 3).cpu().numpy().astype(np.float64)
+        of.run_step(0, 0)
+        torch.cuda.synchronize()
+        planes = [of.debug_plane(0, 4 + f).cpu().numpy().astype(np.float64) for f in range(5)]
+    I2w = oracle.warp(I2, u0, v0)
+    Ix, Iy = oracle.gradients(I1)
+    It = I2w - I1 - Ix * u0 - Iy * v0
+    prods = [Ix * Ix, Ix * Iy, Iy * Iy, Ix * It, Iy * It]
+    w = np.array([oracle.window_weight(t, R, wt) for t in range(-R, R + 1)])
+    sums5 = oracle.iteration(I1, I2, u0, v0, R, wt)[2]
+    for f in range(5):
+        hs = correlate1d(prods[f], w, axis=1, mode="constant", cval=0.0)
+        scale = max(np.abs(hs).max(), 1e-30)
+        assert np.abs(planes[f] - hs).max() <= 1e-5 * scale, (f, np.abs(planes[f] - hs).max(), scale)
+        ws = correlate1d(planes[f], w, axis=0, mode="constant", cval=0.0)
+        scale = max(np.abs(sums5[f]).max(), 1e-30)
+        assert np.abs(ws - sums5[f]).max() <= 1e-5 * scale, (f, np.abs(ws - sums5[f]).max(), scale)
 
 
 def test_single_iteration_kernels_vs_oracle(torch, B, oracle):
@@ -543,3 +579,157 @@ def test_mask_skips_work(torch, B):
         t_half = timed()
     print("solve ms: unmasked %.3f, right half masked %.3f" % (t_full, t_half))
     assert t_half < 0.9 * t_full
+
+
+# ---------------------------------------------------------------------------- conditioning (D14, D15)
+@pytest.mark.parametrize("eps,max_step", [(1e-2, 3.0), (1e-6, 3.0), (1e-3, 0.5)])
+def test_conditioning_parity(torch, B, oracle, eps, max_step):
+    """of_set_conditioning: relative damping 1e-2 / 1e-6 and a step limit of 0.5 px that is active (the images are 2.4 px apart and
+    there is one level, so the first iterations are clamped) against the oracle run with the same constants."""
+    W, H = 224, 160
+    rng = np.random.default_rng(2461)
+    xp, yp, amp = syn.seed_particles(rng, W, H, 0.04, 120, 255)
+    I1 = syn.quantize(syn.render_particles(xp, yp, amp, 1.3, W, H), np.uint8, 255)
+    I2 = syn.quantize(syn.render_particles(xp + 2.4, yp - 1.1, amp, 1.3, W, H), np.uint8, 255)
+    ref = oracle.solve(I1, I2, 1, 9, 5, BOX, eps=eps, max_step=max_step)
+    with B.OpticalFlow(W, H, 1, 9, 5, BOX) as of:
+        of.set_conditioning(eps, max_step)
+        u, v = of.compute(torch.from_numpy(I1).cuda(), torch.from_numpy(I2).cuda())
+        m = of.validity()
+        torch.cuda.synchronize()
+        u, v, m = u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy()
+    st = assert_parity(u, v, m, ref, "conditioning eps=%g max_step=%g" % (eps, max_step))
+    if max_step < 1.0:                                  # the clamp was active: after 5 iterations nothing can exceed 5 x 0.5 px
+        assert np.abs(ref["u"]).max() <= 5 * max_step + 1e-9 and np.abs(u).max() <= 5 * max_step + 1e-4
+        assert np.abs(ref["u"]).max() > 4 * max_step
+    print("conditioning", eps, max_step, st)
+
+
+def test_fp32_frames_of_tiny_gain(torch, B, oracle):
+    """Gain invariance of the fp32 path: the same pair scaled by 1e-6 (fp32 frames of very small gain).  The oracle is gain
+    invariant to 4e-15 (pinned on the CPU side); here the fp32 kernels (approximate reciprocal of a determinant of ~1e-20) must
+    still meet the parity bar and agree with the unscaled run."""
+    c = syn.config2(320, 256)
+    g = np.float32(1e-6)
+    f1, f2 = c.I1.astype(np.float32) * g, c.I2.astype(np.float32) * g
+    ref = oracle.solve(f1, f2, c.levels, c.window_radius, c.iterations, c.window_type)
+    u, v, m, _ = gpu_solve(torch, B, f1, f2, c.levels, c.window_radius, c.iterations, c.window_type)
+    st = assert_parity(u, v, m, ref, "tiny gain")
+    u1, v1, m1, _ = gpu_solve(torch, B, c.I1, c.I2, c.levels, c.window_radius, c.iterations, c.window_type)
+    S = ref["det"] > 1e-3 * ref["det"].max()
+    assert np.abs(u - u1)[S].max() < 1e-3 and np.abs(v - v1)[S].max() < 1e-3 and np.array_equal(m, m1)
+    print("tiny gain", st)
+
+
+# ---------------------------------------------------------------------------- streaming variants
+@pytest.mark.parametrize("dtype_name", ["u16", "f32"])
+def test_stream_device_results_and_validity(torch, B, oracle, dtype_name):
+    """of_stream_* with device-resident results (result_on_host = 0), 16-bit and fp32 frames, CONSECUTIVE mode: every field and its
+    validity plane (of_stream_result_validity: one plane per slot of the result ring) equal the non-streaming call bit for bit."""
+    W, H, n = 320, 256, 5
+    rng = np.random.default_rng(77)
+    xp, yp, amp = syn.seed_particles(rng, W, H, 0.03, 1500, 4095)
+    frames = []
+    for k in range(n):
+        img = syn.render_particles(xp + 0.9 * k, yp + 0.3 * k, amp, 1.4, W, H)
+        frames.append(syn.quantize(img, np.uint16, 4095) if dtype_name == "u16" else img.astype(np.float32))
+    dt = B.OF_DTYPE_U16 if dtype_name == "u16" else B.OF_DTYPE_F32
+    to_dev = (lambda a: torch.from_numpy(a.view(np.int16)).cuda()) if dtype_name == "u16" else (lambda a: torch.from_numpy(a).cuda())
+    args = (W, H, 2, 7, 4, BOX)
+    with B.OpticalFlow(*args) as of, B.OpticalFlow(*args) as of2:
+        of.stream_open(dt, B.OF_STREAM_CONSECUTIVE, False)
+        got = []
+        for k, f in enumerate(frames):
+            slot = of.stream_acquire()
+            slot[...] = f
+            of.stream_submit()
+            if k >= 1:
+                idx, pu, pv = of.stream_result()
+                pm = of.stream_result_validity()
+                assert idx == k - 1 and isinstance(pu, int) and isinstance(pm, int)
+                got.append((B.device_to_numpy(pu, W * H, np.float32).reshape(H, W), B.device_to_numpy(pv, W * H, np.float32).reshape(H, W),
+                            B.device_to_numpy(pm, W * H, np.uint8).reshape(H, W)))
+        of.stream_close()
+        for k in range(n - 1):
+            u2, v2 = of2.compute(to_dev(frames[k]), to_dev(frames[k + 1]))
+            m2 = of2.validity()
+            torch.cuda.synchronize()
+            assert np.array_equal(got[k][0], u2.cpu().numpy()) and np.array_equal(got[k][1], v2.cpu().numpy()), k
+            assert np.array_equal(got[k][2], m2.cpu().numpy()), k
+        ref = oracle.solve(frames[0], frames[1], 2, 7, 4, BOX)
+        print("stream", dtype_name, assert_parity(got[0][0], got[0][1], got[0][2], ref, "stream device results"))
+
+
+def test_stream_consecutive_with_mask_and_equalisation(torch, B, oracle):
+    """CONSECUTIVE mode with an obstacle mask and the eq. 2 pre-filter set: the first frame of a stream takes a separate code path
+    (conversion + pyramid only).  Host results and validity planes against the masked oracle on equalised frames."""
+    W, H, n = 320, 256, 4
+    rng = np.random.default_rng(78)
+    xp, yp, amp = syn.seed_particles(rng, W, H, 0.03, 120, 255)
+    frames = [syn.quantize(syn.render_particles(xp + 0.7 * k, yp - 0.4 * k, amp, 1.3, W, H) + 20.0 * (np.arange(W) / W)[None, :], np.uint8, 255)
+              for k in range(n)]
+    mask = syn.mask_backward_step(W, H)
+    with B.OpticalFlow(W, H, 2, 6, 4, GAUSS) as of:
+        of.set_equalisation(5)
+        of.set_mask(mask)
+        of.stream_open(B.OF_DTYPE_U8, B.OF_STREAM_CONSECUTIVE, True)
+        out = []
+        for k, f in enumerate(frames):
+            slot = of.stream_acquire()
+            slot[...] = f
+            of.stream_submit()
+            if k >= 1:
+                idx, u, v = of.stream_result()
+                out.append((u.copy(), v.copy(), of.stream_result_validity().copy()))
+        of.stream_close()
+    eq = [oracle.equalise(f.astype(np.float64), 5) for f in frames]
+    for k in range(n - 1):
+        ref = oracle.solve(eq[k], eq[k + 1], 2, 6, 4, GAUSS, mask=mask)
+        st = assert_parity(out[k][0], out[k][1], out[k][2], ref, "stream mask+eq pair %d" % k)
+        assert np.all(out[k][0][mask == 0] == 0.0) and np.all(out[k][2][mask == 0] == 0)
+    print("stream mask+eq", st)
+
+
+# ---------------------------------------------------------------------------- masked + hoisted against the oracle
+@pytest.mark.parametrize("W,H,L,R,it,wt", [(256, 256, 4, 10, 3, BOX), (320, 256, 3, 12, 4, GAUSS)])
+def test_masked_hoisted_solve_matches_oracle(torch, B, oracle, W, H, L, R, it, wt):
+    """of_set_hoist together with of_set_mask against the masked oracle (the bitwise hoist test compares with the default kernel only)."""
+    c = syn.config3(W, H)
+    mask = np.ones((H, W), np.uint8)
+    mask[H // 3: H // 2, : W // 2] = 0
+    ref = oracle.solve(c.I1, c.I2, L, R, it, wt, mask=mask)
+    with B.OpticalFlow(W, H, L, R, it, wt) as of:
+        of.set_hoist(True)
+        of.set_mask(mask)
+        u, v = of.compute(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda())
+        m = of.validity()
+        torch.cuda.synchronize()
+        u, v, m = u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy()
+    print("mask+hoist", assert_parity(u, v, m, ref, "mask+hoist"))
+    assert np.all(u[mask == 0] == 0.0) and np.all(m[mask == 0] == 0)
+
+
+def test_fused_and_two_pass_levels_agree_bitwise(torch, B):
+    """of_set_fused (coarse levels iterated inside the CTA, of_fused.cuh) against the two-pass form in the same persistent kernel."""
+    for (W, H, L, R, it, wt) in [(256, 256, 1, 8, 4, BOX), (640, 512, 3, 12, 3, GAUSS), (203, 131, 2, 5, 5, BOX)]:
+        c = syn.config3(W, H)
+        d1, d2 = torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()
+        out = []
+        for fused in (True, False):
+            with B.OpticalFlow(W, H, L, R, it, wt) as of:
+                of.set_fused(fused)
+                u, v = of.compute(d1, d2)
+                m = of.validity()
+                torch.cuda.synchronize()
+                out.append((u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy()))
+        assert all(np.array_equal(a, b) for a, b in zip(out[0], out[1])), (W, H, L, R)
+
+
+def test_misaligned_field_pointers_are_rejected(torch, B):
+    c = syn.config1()
+    with B.OpticalFlow(*c.create_args) as of:
+        d1, d2 = torch.from_numpy(c.I1.astype(np.float32)).cuda(), torch.from_numpy(c.I2.astype(np.float32)).cuda()
+        big = torch.empty(c.width * c.height + 4, dtype=torch.float32, device="cuda")
+        good = torch.empty(c.width * c.height, dtype=torch.float32, device="cuda")
+        rc = B.lib().of_compute(of._h, d1.data_ptr(), d2.data_ptr(), big.data_ptr() + 4, good.data_ptr(), None)
+        assert rc == B.OF_ERR_INVALID_ARG and "aligned" in B.last_error()

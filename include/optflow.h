@@ -187,6 +187,14 @@ int of_field_minmax(of_handle h, const float *field_dev, const uint8_t *valid_de
 /* out_dev[0] = number of available vectors with vx <= threshold, out_dev[1] = number of available vectors. */
 int of_bubble_count(of_handle h, const float *vx_dev, const uint8_t *valid_dev, float threshold,
                     unsigned long long *out_dev, void *stream);
+/* The same two steps with the threshold kept on the device, so that S_bubble of a field needs no host round trip ("this
+ * post-processing ... hidden during copy"; eq. 3):
+ *   of_bubble_threshold: threshold_dev[0] = T_v = 0.5 * (min + max) / n_fields of sum_dev (the running sum of n_fields fields,
+ *                        of_field_accumulate) over the available vectors, formed in fp32;
+ *   of_bubble_count_dev: as of_bubble_count with the threshold read from threshold_dev[0]. */
+int of_bubble_threshold(of_handle h, const float *sum_dev, int n_fields, const uint8_t *valid_dev, float *threshold_dev, void *stream);
+int of_bubble_count_dev(of_handle h, const float *vx_dev, const uint8_t *valid_dev, const float *threshold_dev,
+                        unsigned long long *out_dev, void *stream);
 
 /* Stand-alone single steps (rows a2, a10 of the scope table), dense device buffers. */
 int of_pyramid_down(const float *src, int width, int height, float *dst, void *stream);

@@ -36,6 +36,8 @@ SIGNATURES = {
     "of_set_persistent": (_i, [_vp, _i]),
     "of_set_hoist": (_i, [_vp, _i]),
     "of_set_fused": (_i, [_vp, _i]),
+    "of_bubble_threshold": (_i, [_vp, _vp, _i, _vp, _vp, _vp]),
+    "of_bubble_count_dev": (_i, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "of_stream_result_validity": (_i, [_vp, ctypes.POINTER(ctypes.c_void_p)]),
     "of_solve_timeline": (_i, [_vp, _i, _i, _vp, _i]),
     "of_get_validity": (_i, [_vp, _vp, _vp]),
@@ -233,6 +235,20 @@ class OpticalFlow:
         out = self._torch.empty(2, dtype=self._torch.int64, device=vx.device)
         _check(lib().of_bubble_count(self._h, vx.data_ptr(), valid.data_ptr() if valid is not None else None,
                                      float(threshold), out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    def bubble_threshold(self, total, n_fields, valid=None, stream=None):
+        """Device tensor holding T_v = 0.5 * (min + max) / n_fields of the running sum `total` over the available vectors."""
+        out = self._torch.empty(1, dtype=self._torch.float32, device=total.device)
+        _check(lib().of_bubble_threshold(self._h, total.data_ptr(), int(n_fields), valid.data_ptr() if valid is not None else None,
+                                         out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    def bubble_count_dev(self, vx, threshold_dev, valid=None, stream=None):
+        """As bubble_count with the threshold taken from a device tensor (no host round trip)."""
+        out = self._torch.empty(2, dtype=self._torch.int64, device=vx.device)
+        _check(lib().of_bubble_count_dev(self._h, vx.data_ptr(), valid.data_ptr() if valid is not None else None,
+                                         threshold_dev.data_ptr(), out.data_ptr(), _stream_ptr(stream)))
         return out
 
     # -- frame pipeline -----------------------------------------------------------------------

@@ -56,10 +56,15 @@ __global__ void __launch_bounds__(256) kp_minmax(const float *__restrict__ f, co
 
 __global__ void kp_minmax_finish(const unsigned *mm, float *out) { out[0] = ord2f(mm[0]); out[1] = ord2f(mm[1]); }
 
+// T_v = (min + max) / 2 of the MEAN field from the min / max of the running SUM of n fields, in fp32: 0.5f * (lo + hi) / n
+__global__ void kp_threshold_finish(const unsigned *mm, float n_fields, float *out) { out[0] = 0.5f * (ord2f(mm[0]) + ord2f(mm[1])) / n_fields; }
+
 // cnt[0] = available vectors with vx <= threshold, cnt[1] = available vectors (cnt zeroed before the launch)
+// (threshold_dev != NULL: the threshold is read from device memory, so that no step of eq. 3 needs the host)
 __global__ void __launch_bounds__(256) kp_bubble_count(const float *__restrict__ vx, const uint8_t *__restrict__ valid, size_t n,
-                                                       float threshold, unsigned long long *cnt)
+                                                       float threshold, const float *__restrict__ threshold_dev, unsigned long long *cnt)
 {
+    if (threshold_dev != nullptr) threshold = threshold_dev[0];
     unsigned below = 0, total = 0;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {

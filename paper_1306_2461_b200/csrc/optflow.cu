@@ -1094,7 +1094,30 @@ int of_bubble_count(of_handle h, const float *vx_dev, const uint8_t *valid_dev, 
     const size_t n = (size_t)h->W * h->H;
     cudaStream_t st = (cudaStream_t)stream;
     CU_TRY(cudaMemsetAsync(out_dev, 0, 2 * sizeof(unsigned long long), st));
-    kp_bubble_count<<<2 * h->sms, 256, 0, st>>>(vx_dev, valid_dev, n, threshold, out_dev);
+    kp_bubble_count<<<2 * h->sms, 256, 0, st>>>(vx_dev, valid_dev, n, threshold, nullptr, out_dev);
+    CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+int of_bubble_threshold(of_handle h, const float *sum_dev, int n_fields, const uint8_t *valid_dev, float *threshold_dev, void *stream)
+{
+    if (!h || !sum_dev || !threshold_dev || n_fields < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    const size_t n = (size_t)h->W * h->H;
+    cudaStream_t st = (cudaStream_t)stream;
+    kp_minmax_init<<<1, 1, 0, st>>>(h->d_post);
+    kp_minmax<<<2 * h->sms, 256, 0, st>>>(sum_dev, valid_dev, n, h->d_post);
+    kp_threshold_finish<<<1, 1, 0, st>>>(h->d_post, (float)n_fields, threshold_dev);
+    CU_TRY(cudaGetLastError());
+    return OF_OK;
+}
+
+int of_bubble_count_dev(of_handle h, const float *vx_dev, const uint8_t *valid_dev, const float *threshold_dev, unsigned long long *out_dev, void *stream)
+{
+    if (!h || !vx_dev || !out_dev || !threshold_dev) return fail(OF_ERR_INVALID_ARG, "null argument");
+    const size_t n = (size_t)h->W * h->H;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(cudaMemsetAsync(out_dev, 0, 2 * sizeof(unsigned long long), st));
+    kp_bubble_count<<<2 * h->sms, 256, 0, st>>>(vx_dev, valid_dev, n, 0.f, threshold_dev, out_dev);
     CU_TRY(cudaGetLastError());
     return OF_OK;
 }

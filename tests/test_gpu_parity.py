@@ -493,6 +493,12 @@ def test_bubble_surface_counts_match_oracle_exactly(torch, B, oracle):
         assert tuple(cnt.cpu().tolist()) == oracle.bubble_counts(fields[2].cpu().numpy(), float(T), mh)
         assert tuple(cnt_all.cpu().tolist()) == oracle.bubble_counts(fields[2].cpu().numpy(), float(T))
         assert 0 < cnt[0] < cnt[1] <= W * H
+        # the same with the threshold kept on the device (no host value between the steps of eq. 3)
+        thr_dev = of.bubble_threshold(total, 3, m)
+        cnt_dev = of.bubble_count_dev(fields[2], thr_dev, m)
+        torch.cuda.synchronize()
+        assert np.float32(thr_dev.cpu().numpy()[0]) == T
+        assert tuple(cnt_dev.cpu().tolist()) == tuple(cnt.cpu().tolist())
 
 
 # ---------------------------------------------------------------------------- NEXT item f4: obstacle masks

@@ -17,6 +17,7 @@
 #pragma once
 #include "of_k2.cuh"
 #include "of_k3.cuh"
+#include <type_traits>
 
 template <int R> struct FusedGeom {
     static constexpr int RL = K2Geom<R>::RL, OFF = K2Geom<R>::OFF, NIN = K2Geom<R>::NIN;
@@ -65,23 +66,26 @@ __device__ __forceinline__ void fused_vsolve(const FusedParams &p, const K3Param
             uu[j] = !p.zero_uv ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
             vv[j] = !p.zero_uv ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
         }
-        float2 acc[5][SEG];
+        float2 acc[5][SEG], core[5];
 #pragma unroll
-        for (int f = 0; f < 5; ++f)
+        for (int f = 0; f < 5; ++f) {
+            core[f] = make_float2(0.f, 0.f);
 #pragma unroll
             for (int j = 0; j < SEG; ++j) acc[f][j] = make_float2(0.f, 0.f);
-        // summed row r of the task is image row gy0 - R + r = buffer row SEG*rb + (RT - R) + r; taps top to bottom as in k3_phase
-        const float *col = hs + (size_t)(SEG * rb + (G::RT - R)) * tw + 2 * c;
-#pragma unroll
-        for (int r = 0; r < SEG + 2 * R; ++r) {
-#pragma unroll
-            for (int f = 0; f < 5; ++f) {
-                const float2 val = *reinterpret_cast<const float2 *>(col + (size_t)(f * PH + r) * tw);
-#pragma unroll
-                for (int j = 0; j < SEG; ++j)
-                    if (r - j >= 0 && r - j <= 2 * R) acc[f][j] = fma2s(p.ww.w[r - j], val, acc[f][j]);
-            }
         }
+        // summed row r of the task is image row gy0 - R + r = buffer row SEG*rb + (RT - R) + r; rows top to bottom as in k3_phase
+        const float *col = hs + (size_t)(SEG * rb + (G::RT - R)) * tw + 2 * c;
+        auto sum_rows = [&](auto box) {
+            constexpr bool BOX = decltype(box)::value;
+#pragma unroll
+            for (int r = 0; r < SEG + 2 * R; ++r)
+#pragma unroll
+                for (int f = 0; f < 5; ++f)
+                    win_vrow<R, SEG, BOX>(p.ww, r, *reinterpret_cast<const float2 *>(col + (size_t)(f * PH + r) * tw), acc[f], core[f]);
+#pragma unroll
+            for (int f = 0; f < 5; ++f) win_vfinish<SEG, BOX>(acc[f], core[f]);
+        };
+        if (win_box_path(R) && p.ww.box) sum_rows(std::true_type()); else sum_rows(std::false_type());
         k3_solve_store<false, SEG>(p3, acc, uu, vv, mk, gx, gy0, nrows);
     }
 }
@@ -170,13 +174,7 @@ __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned c
                 in[2 * q + 1] = make_float2(v4.z, v4.w);
             }
             float2 acc[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) acc[j] = make_float2(0.f, 0.f);
-#pragma unroll
-            for (int i = 0; i < G::NIN; ++i)
-#pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    if (i - j - G::OFF >= 0 && i - j - G::OFF <= 2 * R) acc[j] = fma2s(p.ww.w[i - j - G::OFF], in[i], acc[j]);
+            win_hsum8<R, G::OFF, G::NIN>(p.ww, in, acc);
             float *d0 = hs + (size_t)(f * PH + 2 * rp) * tw + 8 * sg;
             *reinterpret_cast<float4 *>(d0) = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);
             *reinterpret_cast<float4 *>(d0 + 4) = make_float4(acc[4].x, acc[5].x, acc[6].x, acc[7].x);

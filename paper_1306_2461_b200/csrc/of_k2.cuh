@@ -310,21 +310,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
                     in[2 * k + 1] = make_float2(q.z, q.w);
                 }
                 float2 acc[8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) acc[j] = make_float2(0.f, 0.f);
-                // input-major: one input pair feeds up to eight independent accumulators (same order of taps per output)
-#ifdef K2_TAP_MAJOR
-#pragma unroll
-                for (int tap = 0; tap <= 2 * R; ++tap)
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) acc[j] = fma2s(p.ww.w[tap], in[j + tap + G::OFF], acc[j]);
-#else
-#pragma unroll
-                for (int i = 0; i < G::NIN; ++i)
-#pragma unroll
-                    for (int j = 0; j < 8; ++j)
-                        if (i - j - G::OFF >= 0 && i - j - G::OFF <= 2 * R) acc[j] = fma2s(p.ww.w[i - j - G::OFF], in[i], acc[j]);
-#endif
+                win_hsum8<R, G::OFF, G::NIN>(p.ww, in, acc);
                 if (gx < pitch && !OF_DBG(p.dbg, 32)) {
                     float *d0 = p.S + f * p.plane + (size_t)gy * pitch + gx;
                     if (gy < H) {

@@ -368,14 +368,7 @@ __device__ __forceinline__ void k2s_hsum_task(const K2SParams &p, const K2SSmem<
             in[2 * k + 1] = make_float2(v.z, v.w);
         }
         float2 acc[8];
-#pragma unroll
-        for (int jj = 0; jj < 8; ++jj) acc[jj] = make_float2(0.f, 0.f);
-        // input-major: one input pair feeds up to eight independent accumulators; taps of an output are added left to right
-#pragma unroll
-        for (int i = 0; i < G::NIN; ++i)
-#pragma unroll
-            for (int jj = 0; jj < 8; ++jj)
-                if (i - jj - G::OFF >= 0 && i - jj - G::OFF <= 2 * R) acc[jj] = fma2s(p.ww.w[i - jj - G::OFF], in[i], acc[jj]);
+        win_hsum8<R, G::OFF, G::NIN>(p.ww, in, acc);
         if (gx < p.pitch) {
             float *d0 = p.S + f * p.plane + (size_t)gy * p.pitch + gx;
             if (gy < p.H) {

@@ -22,6 +22,7 @@
 #pragma once
 #include "of_common.cuh"
 #include "of_async.cuh"
+#include <type_traits>
 
 #ifndef K3_SEG
 #define K3_SEG 4                                          // rows per task = rows per TMA chunk (4: finer tasks, better
@@ -283,22 +284,28 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             fb[k] = full0 + 8 * slot;
             fpar[k] = (gc / K3_RING) & 1;
         }
-        float2 acc[5][K3_SEG];
+        float2 acc[5][K3_SEG], core[5];
 #pragma unroll
-        for (int f = 0; f < 5; ++f)
+        for (int f = 0; f < 5; ++f) {
+            core[f] = make_float2(0.f, 0.f);
 #pragma unroll
             for (int j = 0; j < K3_SEG; ++j) acc[f][j] = make_float2(0.f, 0.f);
-        if (!OF_DBG(p.dbg, 2))
+        }
+        auto sum_rows = [&](auto box) {
+            constexpr bool BOX = decltype(box)::value;
 #pragma unroll
-        for (int r = 0; r < G::NIN; ++r) {
-            if ((r % K3_SEG) == 0 && !OF_DBG(p.dbg, 1)) mbar_wait(fb[r / K3_SEG], fpar[r / K3_SEG]);   // chunk by chunk, as the TMA delivers them
+            for (int r = 0; r < G::NIN; ++r) {
+                if ((r % K3_SEG) == 0 && !OF_DBG(p.dbg, 1)) mbar_wait(fb[r / K3_SEG], fpar[r / K3_SEG]);   // chunk by chunk, as the TMA delivers them
 #pragma unroll
-            for (int f = F0; f < 5; ++f) {
-                const float2 val = *reinterpret_cast<const float2 *>(cb[r / K3_SEG] + (f - F0) * (K3_SEG * 256) + (r % K3_SEG) * 256);
-#pragma unroll
-                for (int j = 0; j < K3_SEG; ++j)
-                    if (r - j >= 0 && r - j <= 2 * R) acc[f][j] = fma2s(p.ww.w[r - j], val, acc[f][j]);
+                for (int f = F0; f < 5; ++f)
+                    win_vrow<R, K3_SEG, BOX>(p.ww, r, *reinterpret_cast<const float2 *>(cb[r / K3_SEG] + (f - F0) * (K3_SEG * 256) + (r % K3_SEG) * 256),
+                                             acc[f], core[f]);
             }
+#pragma unroll
+            for (int f = F0; f < 5; ++f) win_vfinish<K3_SEG, BOX>(acc[f], core[f]);
+        };
+        if (!OF_DBG(p.dbg, 2)) {
+            if (win_box_path(R) && p.ww.box) sum_rows(std::true_type()); else sum_rows(std::false_type());
         }
         __syncwarp();
         if (lane == 0 && !OF_DBG(p.dbg, 1)) {

@@ -786,6 +786,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     c->last_done = nullptr; c->last_stream = nullptr; c->have_last = false; c->bench_out = nullptr;
     memcpy(c->lv, lv, sizeof lv);
     memset(&c->ww, 0, sizeof c->ww);
+    c->ww.box = window_type == OF_WINDOW_BOX ? 1 : 0;
     for (int t = -window_radius; t <= window_radius; ++t) {
         double w = 1.0;
         if (window_type == OF_WINDOW_GAUSSIAN) {

@@ -739,3 +739,33 @@ def test_misaligned_field_pointers_are_rejected(torch, B):
         good = torch.empty(c.width * c.height, dtype=torch.float32, device="cuda")
         rc = B.lib().of_compute(of._h, d1.data_ptr(), d2.data_ptr(), big.data_ptr() + 4, good.data_ptr(), None)
         assert rc == B.OF_ERR_INVALID_ARG and "aligned" in B.last_error()
+
+
+@pytest.mark.parametrize("W,H,L,R,it,wt,hoist,masked", [(320, 256, 3, 12, 4, GAUSS, False, False), (256, 256, 1, 8, 4, BOX, False, False),
+                                                        (448, 320, 2, 7, 6, BOX, True, True), (1280, 1024, 3, 12, 10, GAUSS, False, False)])
+def test_repeated_solves_are_bitwise_stable(torch, B, W, H, L, R, it, wt, hoist, masked):
+    """Race evidence without a sanitizer (compute-sanitizer is closed on this GPU pool, profiles/r2_sanitizer.md): the grid barrier,
+    the mbarrier rings, the proxy fences and the shared-memory union between the passes are all exercised by 60 back-to-back solves on
+    one handle, alternating two different pairs, and every result must reproduce the first one of its pair bit for bit."""
+    ca, cb = syn.config3(W, H, seed_offset=0), syn.config3(W, H, seed_offset=1)
+    d = [(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()) for c in (ca, cb)]
+    with B.OpticalFlow(W, H, L, R, it, wt) as of:
+        of.set_hoist(hoist)
+        if masked:
+            mask = np.ones((H, W), np.uint8)
+            mask[H // 3: H // 2, : W // 2] = 0
+            of.set_mask(mask)
+        first = [None, None]
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            outs = []
+            for k in range(60):
+                u, v = of.compute(d[k & 1][0], d[k & 1][1])
+                outs.append((k & 1, u, v, of.validity()))
+        s.synchronize()
+        for k, u, v, m in outs:
+            if first[k] is None:
+                first[k] = (u, v, m)
+            else:
+                assert torch.equal(u, first[k][0]) and torch.equal(v, first[k][1]) and torch.equal(m, first[k][2])
+        assert not torch.equal(first[0][0], first[1][0])

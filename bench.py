@@ -46,8 +46,8 @@ WORKLOADS = {
                 "10 iterations, frames uploaded from host memory through the pinned double-buffered pipeline"),
 }
 RING = 16          # default: distinct input pairs + output buffers cycled through: 16*(2.6+10.5) MB = 210 MB > 126 MB L2 (config 3)
-DRAM_FILE = os.path.join(ROOT, "profiles", "r2_solve_dram.json")     # dram__bytes of one solve launch per workload, from the ncu captures
-L2_STREAM_GBPS = 14600.0   # measured: a plain streaming kernel with the K2 byte mix (4 planes read, 5 written, 47 MB, L2 resident) on this B200 (profiles/r2_l2_fabric.md)
+DRAM_FILE = os.path.join(ROOT, "profiles", "r2_solve_dram.csv")      # dram__bytes of one solve launch per workload, from the ncu captures
+L2_STREAM_GBPS = 14600.0   # measured: a plain streaming kernel with the K2 byte mix (4 planes read, 5 written, 47 MB, L2 resident) on this B200 (profiles/r2_notes.md)
 
 
 def measured_peaks():
@@ -63,10 +63,13 @@ def measured_peaks():
 def ncu_dram_bytes(workload):
     """dram__bytes_read.sum + dram__bytes_write.sum of one solve launch, as captured with ncu for this build (profiles/)."""
     try:
-        d = json.load(open(DRAM_FILE)).get(workload)
-        return (float(d["dram_bytes"]), d.get("source", DRAM_FILE)) if d else (None, None)
+        import csv
+        for row in csv.DictReader(open(DRAM_FILE)):
+            if row["workload"] == workload:
+                return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), row["source"]
     except Exception:
-        return None, None
+        pass
+    return None, None
 
 
 class ClockSampler:
@@ -414,6 +417,18 @@ def run_ours(args):
         iter_us = float(med.sum())
         iter_gbs = 72.0 * px / (iter_us * 1e-6) / 1e9
         value = world * args.steps / (ms * 1e-3)
+        # every level, coarse to fine (a fused coarse level has one pass and one barrier per iteration: its time is under k2_pass)
+        levels_tl, k = [], 0
+        for l in range(L - 1, -1, -1):
+            if l < L - 1:
+                levels_tl.append({"level": l, "hand_down_us": float(d[k]), "hand_down_barrier_us": float(d[k + 1])})
+                k += 2
+            sg = d[k:k + 4 * it].reshape(it, 4)
+            k += 4 * it
+            m4 = np.median(sg[:-1], axis=0) if it > 1 else sg[0]
+            levels_tl.append({"level": l, "pixels": level_px[l], "k2_pass_us": float(m4[0]), "barrier_1_us": float(m4[1]), "k3_pass_us": float(m4[2]),
+                              "barrier_2_us": float(m4[3]), "iteration_us": float(m4.sum()),
+                              "frac_of_peak": 72.0 * level_px[l] / (float(m4.sum()) * 1e-6) / 1e9 / peak})
         hoist_out = None
         if hoist is not None:
             h_ms, h_solve_us, h_tl = hoist
@@ -462,6 +477,7 @@ def run_ours(args):
             "iteration_level0": {"bytes": 72 * px, "us": iter_us, "GB/s": iter_gbs, "frac_of_peak": iter_gbs / peak,
                                  "phases_us": {"k2_pass": float(med[0]), "barrier_1": float(med[1]), "k3_pass": float(med[2]), "barrier_2": float(med[3])},
                                  "how": "in-kernel SM cycle stamps (of_solve_timeline, max over CTAs) / sampled SM clock; median over iterations"},
+            "levels_timeline": levels_tl,
             "variant_hoist": hoist_out,
             "cpu_baseline": cpu,
             "cpu_baseline_1thread": cpu1,

@@ -30,8 +30,9 @@ __host__ __device__ __forceinline__ void cta_range(int n, int cta, int ncta, int
 // packed fp32 pair FMA with a scalar weight (FFMA2 on sm_100a: half the issue slots of two FFMA)
 __device__ __forceinline__ float2 fma2s(float w, float2 x, float2 acc) { return __ffma2_rn(x, make_float2(w, w), acc); }
 
-// ---- window sums (D11, D12).  Two forms, chosen by ww.box (uniform over the launch), shared by K2, K3 and the fused
-// coarse-level pass so that every caller forms a sum with the same instructions:
+// ---- window sums (D11, D12).  Two forms, chosen at COMPILE time (template parameter BX of the kernels: a kernel that
+// carried both forms was 9500 instructions long and lost 3-7 % to instruction fetches), shared by K2, K3 and the fused coarse-level
+// pass so that every caller forms a sum with the same instructions:
 //   * weighted (Gaussian, and boxes of radius < 4): direct (2R+1)-tap sums, taps in ascending order, one FFMA2 per tap;
 //   * box, R >= 4: the outputs of a lane share most of their taps, so the shared CORE is summed once and every output adds its few
 //     private taps: add-only (no "add the entering value, subtract the leaving one"), hence no cancellation, a sum of non-negative
@@ -40,10 +41,11 @@ __device__ __forceinline__ float2 fma2s(float w, float2 x, float2 acc) { return 
 __host__ __device__ constexpr bool win_box_path(int R) { return R >= 4; }
 
 // Horizontal: 8 adjacent outputs (x 2 rows, packed) of one field from NIN inputs; output j sums in[j+OFF .. j+OFF+2R].
-template <int R, int OFF, int NIN>
+template <int R, int OFF, int NIN, bool BX>
 __device__ __forceinline__ void win_hsum8(const WinWeights &ww, const float2 (&in)[NIN], float2 (&acc)[8])
 {
-    if (win_box_path(R) && ww.box) {
+    static_assert(!BX || win_box_path(R), "the add-only path needs R >= 4");
+    if (BX) {
         float2 core = in[7 + OFF];                                       // taps 7+OFF .. OFF+2R belong to all eight outputs
 #pragma unroll
         for (int k = 8 + OFF; k <= OFF + 2 * R; ++k) core = __fadd2_rn(core, in[k]);

@@ -18,6 +18,20 @@
     default: break;                                                                                \
     }
 
+// Radius and window form: CALL sees `constexpr int R` and `constexpr bool BX` (BX only for box windows of radius >= 4, of_common.cuh).
+#define DISPATCH_RB_CASE(N, BOX_, CALL)                                                            \
+    case N: { constexpr int R = N;                                                                 \
+              if ((BOX_) && win_box_path(N)) { constexpr bool BX = win_box_path(N); CALL; }        \
+              else { constexpr bool BX = false; CALL; } } break;
+#define DISPATCH_RB(R_, BOX_, CALL)                                                                \
+    switch (R_) {                                                                                  \
+    DISPATCH_RB_CASE(1, BOX_, CALL) DISPATCH_RB_CASE(2, BOX_, CALL) DISPATCH_RB_CASE(3, BOX_, CALL) DISPATCH_RB_CASE(4, BOX_, CALL)     \
+    DISPATCH_RB_CASE(5, BOX_, CALL) DISPATCH_RB_CASE(6, BOX_, CALL) DISPATCH_RB_CASE(7, BOX_, CALL) DISPATCH_RB_CASE(8, BOX_, CALL)     \
+    DISPATCH_RB_CASE(9, BOX_, CALL) DISPATCH_RB_CASE(10, BOX_, CALL) DISPATCH_RB_CASE(11, BOX_, CALL) DISPATCH_RB_CASE(12, BOX_, CALL)  \
+    DISPATCH_RB_CASE(13, BOX_, CALL) DISPATCH_RB_CASE(14, BOX_, CALL) DISPATCH_RB_CASE(15, BOX_, CALL) DISPATCH_RB_CASE(16, BOX_, CALL) \
+    default: break;                                                                                \
+    }
+
 // optflow_hoist.cu: of_solve_pair<R, false, true>; forwards to optflow_hoist_mask.cu (of_solve_pair<R, true, true>) when mk is set.
 // Launch (cooperative, `sms` CTAs) and one-time attribute set-up (both units).
 cudaError_t of_launch_solve_hoisted(int R, bool mk, const SolveArgs &a, int sms, cudaStream_t st);

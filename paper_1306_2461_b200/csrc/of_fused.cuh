@@ -45,7 +45,7 @@ struct FusedParams {
 };
 
 // Vertical window sums + solve + update of one tile out of the horizontally summed rows `hs` ([field][PH rows][tw]).
-template <int R, int SEG>
+template <int R, int SEG, bool BX>
 __device__ __forceinline__ void fused_vsolve(const FusedParams &p, const K3Params &p3, const float *hs, int x0, int y0, int tid, int nthr)
 {
     typedef FusedGeom<R> G;
@@ -85,7 +85,7 @@ __device__ __forceinline__ void fused_vsolve(const FusedParams &p, const K3Param
 #pragma unroll
             for (int f = 0; f < 5; ++f) win_vfinish<SEG, BOX>(acc[f], core[f]);
         };
-        if (win_box_path(R) && p.ww.box) sum_rows(std::true_type()); else sum_rows(std::false_type());
+        sum_rows(std::integral_constant<bool, BX>());
         k3_solve_store<false, SEG>(p3, acc, uu, vv, mk, gx, gy0, nrows);
     }
 }
@@ -93,7 +93,7 @@ __device__ __forceinline__ void fused_vsolve(const FusedParams &p, const K3Param
 // One iteration of a level by the CTAs of the grid: CTA `cta` runs tiles cta, cta + ncta, ...  All threads of the CTA take part;
 // `smem` is the CTA's dynamic shared memory (at least FusedGeom<R>::smem_bytes(tw, th) bytes).
 // (__forceinline__ on purpose: as a __noinline__ function it spills and costs 4 us per iteration.)
-template <int R>
+template <int R, bool BX>
 __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned char *smem, int cta, int ncta)
 {
     typedef FusedGeom<R> G;
@@ -174,7 +174,7 @@ __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned c
                 in[2 * q + 1] = make_float2(v4.z, v4.w);
             }
             float2 acc[8];
-            win_hsum8<R, G::OFF, G::NIN>(p.ww, in, acc);
+            win_hsum8<R, G::OFF, G::NIN, BX>(p.ww, in, acc);
             float *d0 = hs + (size_t)(f * PH + 2 * rp) * tw + 8 * sg;
             *reinterpret_cast<float4 *>(d0) = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);
             *reinterpret_cast<float4 *>(d0 + 4) = make_float4(acc[4].x, acc[5].x, acc[6].x, acc[7].x);
@@ -184,7 +184,7 @@ __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned c
         __syncthreads();
         // ---------------- vertical window sums + solve + update: lane task = 2 columns x K3_SEG rows (shorter tasks on small tiles, so
         // that every thread has one, were measured slower: 14.2 against 12.5 us per iteration at 640x512)
-        fused_vsolve<R, K3_SEG>(p, p3, hs, x0, y0, tid, nthr);
+        fused_vsolve<R, K3_SEG, BX>(p, p3, hs, x0, y0, tid, nthr);
         __syncthreads();                                   // the buffers are reused by the CTA's next tile
     }
 }

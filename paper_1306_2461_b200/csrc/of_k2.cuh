@@ -22,6 +22,9 @@
 #ifndef K2_AHEAD_MIN_ROUNDS
 #define K2_AHEAD_MIN_ROUNDS 2                      // tiles with more product rounds than this request u, v of all rounds up front
 #endif
+#ifndef K2_AHEAD_MAX_ROUNDS
+#define K2_AHEAD_MAX_ROUNDS 5                      // ... and at most this many (32 segments of 8 columns + halo = 140 tasks)
+#endif
 #ifndef K2_MAX_WARPS
 #define K2_MAX_WARPS 12                            // warps per CTA (independent of each other); runtime blockDim
 #endif
@@ -198,7 +201,7 @@ template <bool MK> __device__ __forceinline__ void k2_task_products(const K2Para
 // MK = an obstacle mask is set (p.mask and p.list are valid): a separate instantiation, so that the unmasked
 // path carries none of the mask's instructions or registers.
 // HO = of_set_hoist: p.f_first selects the planes formed (0 otherwise, at compile time).
-template <int R, bool MK, bool HO>
+template <int R, bool MK, bool HO, bool BX>
 __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_cta, int *tile_counter, int warp, int lane, int t_begin, int t_end)
 {
     typedef K2Geom<R> G;
@@ -226,13 +229,14 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
         // ---------------- phase 1: products of (PW x TH) pixels -> shared memory
         // task k -> (row pair rp, column pair cp): input loads, then the 16 gathers of its four pixels,
         // then the arithmetic (other warps of the SM cover the two memory latencies)
-        if (ntasks > 32 * K2_AHEAD_MIN_ROUNDS) {
+        if (ntasks > 32 * K2_AHEAD_MIN_ROUNDS && ntasks <= 32 * K2_AHEAD_MAX_ROUNDS) {
         // wide tiles (three or more product rounds): the field values of ALL rounds of the tile are requested first, so that a
         // round's gathers wait for one L2 round trip (I1 / I2) instead of two (u, v, then I2).  Measured (profiles/r1_experiments.md):
         // level-0 K2 pass 16.0 -> 15.1 us at 1280x1024, 57.2 -> 50.1 us at 2048x2048; one-round tiles of the coarse levels lose
         // 0.4 us with it (unrolled guards), so they keep the rolled loop below.
-        constexpr int MAXR = 6;                            // product rounds of the widest tile: (nseg <= 32: 128 + RL column pairs) / 32
-        static_assert(128 + 4 * G::RL <= 32 * MAXR, "MAXR too small for the widest warp tile");
+        constexpr int MAXR = K2_AHEAD_MAX_ROUNDS;          // (wider tiles take the rolled loop below.  Every unrolled round is ~350 instructions
+                                                           // and the kernel is sensitive to its code size: 6 -> 5 rounds gave the hoisted kernel 7 %.
+                                                           // One rolled loop with the requested values moved down a place per round was slower.)
         float2 pu0[MAXR], pu1[MAXR], pv0[MAXR], pv1[MAXR];
 #pragma unroll
         for (int r = 0; r < MAXR; ++r) {
@@ -310,7 +314,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
                     in[2 * k + 1] = make_float2(q.z, q.w);
                 }
                 float2 acc[8];
-                win_hsum8<R, G::OFF, G::NIN>(p.ww, in, acc);
+                win_hsum8<R, G::OFF, G::NIN, BX>(p.ww, in, acc);
                 if (gx < pitch && !OF_DBG(p.dbg, 32)) {
                     float *d0 = p.S + f * p.plane + (size_t)gy * pitch + gx;
                     if (gy < H) {
@@ -328,7 +332,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
     }
 }
 
-template <int R, bool MK>
+template <int R, bool MK, bool BX>
 __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K2Params p)
 {
     extern __shared__ float4 smem4[];                          // warp slices, then 16 bytes for the tile counter
@@ -338,5 +342,5 @@ __global__ void __launch_bounds__(32 * K2_MAX_WARPS, 1) k2_products_hsum(const K
     __syncthreads();
     int t_begin, t_end;
     cta_range(p.ntiles, blockIdx.x, gridDim.x, t_begin, t_end);
-    k2_phase<R, MK, false>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, t_begin, t_end);
+    k2_phase<R, MK, false, BX>(p, reinterpret_cast<unsigned char *>(smem4), tile_counter, threadIdx.x >> 5, threadIdx.x & 31, t_begin, t_end);
 }

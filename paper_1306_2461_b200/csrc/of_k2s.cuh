@@ -53,7 +53,7 @@ template <int R> struct K2S {
     static constexpr int WROWS = RU + 2 * HYR + 1;                             // rows of a unit's I2 window: y0-HYR .. y0+RU+HYR
     static constexpr int WPAD = (WROWS + RU - 1) / RU * RU - WROWS;            // extra rows on top of a run's first window (whole boxes)
     static constexpr int I2BOX_BYTES = RU * PWB * 4;
-    static constexpr int NB = 11, NU = 2 * NB, D = 6, LAG = 2;                 // product buffers; unit slots of the barriers; prefetch distance; P-to-H lag
+    static constexpr int NB = 11, NU = 2 * NB, LAG = 2;                 // product buffers; unit slots of the barriers (> NGRP + LU: never the limit of the run-ahead); P-to-H lag
     static constexpr int DATA_MAX = 225280;                                    // bytes below the barrier area (= the K3 ring, of_k3.cuh)
     static constexpr int NBOX0 = (WROWS + WPAD) / RU;                          // boxes of a run's first window
     static constexpr int LU = (2 * HYR + RU) / RU;                             // a box loaded for unit i is last read by unit i + LU
@@ -141,7 +141,10 @@ __device__ __forceinline__ void k2s_produce(const K2SParams &p, const K2SSmem<R>
     for (int ip = 0; ip < n; ++ip) {
         const bool new_run = (ip == 0) || (j == 0);
         const int nbox = new_run ? G::NBOX0 : 1;
-        int m = ip - G::NU;                          // the descriptor / barrier slot of unit ip - NU
+        // the descriptor / barrier slot of unit ip - NU is re-used: the product tasks of the units ip - NU .. ip - NU + LU wait on
+        // that mbarrier (their windows hold rows copied for it) and must all be past their wait before it starts another phase:
+        // an mbarrier only tells the parity of its current phase, so a waiter that is two phases late would wait for ever
+        int m = ip - G::NU + G::LU;
         {
             int g2 = gi;
             for (int b = 0; b < nbox; ++b) { m = max(m, sm.last_user[g2]); g2 = g2 + 1 == G::NGRP ? 0 : g2 + 1; }
@@ -344,7 +347,7 @@ __device__ __forceinline__ void k2s_products_task(const K2SParams &p, const K2SS
 
 // ---------------------------------------------------------------------------------------------------------------- H task
 // Field f of unit g (or nothing, `skip`: a plane this pass does not form): horizontal window sums from the product buffer to the plane.
-template <int R>
+template <int R, bool BX>
 __device__ __forceinline__ void k2s_hsum_task(const K2SParams &p, const K2SSmem<R> &sm, int lane, int g, uint32_t q, int f, bool skip, long long *prof)
 {
     typedef K2S<R> G;
@@ -368,7 +371,7 @@ __device__ __forceinline__ void k2s_hsum_task(const K2SParams &p, const K2SSmem<
             in[2 * k + 1] = make_float2(v.z, v.w);
         }
         float2 acc[8];
-        win_hsum8<R, G::OFF, G::NIN>(p.ww, in, acc);
+        win_hsum8<R, G::OFF, G::NIN, BX>(p.ww, in, acc);
         if (gx < p.pitch) {
             float *d0 = p.S + f * p.plane + (size_t)gy * p.pitch + gx;
             if (gy < p.H) {
@@ -390,7 +393,7 @@ __device__ __forceinline__ void k2s_hsum_task(const K2SParams &p, const K2SSmem<
 // ---------------------------------------------------------------------------------------------------------------- the pass
 // One K2 pass over a level by the CTA that owns units [u_begin, u_end).  Warps 0 .. K2S_WORKERS-1 work, warp K2S_WORKERS produces.
 // *sm.ticket must be 0 on entry (CTA-synchronised); the caller resets it after the pass and adds u_end - u_begin to `ub`.
-template <int R, bool HO>
+template <int R, bool HO, bool BX>
 __device__ __forceinline__ void k2s_phase(const K2SParams &p, const K2SSmem<R> &sm, int warp, int lane, int u_begin, int u_end, uint32_t ub)
 {
     typedef K2S<R> G;
@@ -421,7 +424,7 @@ __device__ __forceinline__ void k2s_phase(const K2SParams &p, const K2SSmem<R> &
             if (i < n) k2s_products_task<R, HO>(p, sm, lane, u_begin + i, ub + (uint32_t)i, kind, in, prof);
         } else {
             const int ih = i - G::LAG, f = kind - G::NROUND;
-            if (ih >= 0 && ih < n) k2s_hsum_task<R>(p, sm, lane, u_begin + ih, ub + (uint32_t)ih, f, f < f_first, prof);
+            if (ih >= 0 && ih < n) k2s_hsum_task<R, BX>(p, sm, lane, u_begin + ih, ub + (uint32_t)ih, f, f < f_first, prof);
         }
     };
     K2In in_a = {}, in_b = {};
@@ -452,7 +455,7 @@ __device__ __forceinline__ void k2s_phase(const K2SParams &p, const K2SSmem<R> &
 }
 
 // Stand-alone launch of one K2 pass (of_set_persistent(0), of_run_step): the same pass function as in the persistent solve kernel.
-template <int R>
+template <int R, bool BX>
 __global__ void __launch_bounds__(32 * (K2S_WORKERS + 1), 1) k2s_products_hsum(const K2SParams p)
 {
     extern __shared__ __align__(1024) unsigned char k2s_smem_[];
@@ -464,5 +467,5 @@ __global__ void __launch_bounds__(32 * (K2S_WORKERS + 1), 1) k2s_products_hsum(c
     __syncthreads();
     int ub, ue;
     cta_range(p.nunits, blockIdx.x, gridDim.x, ub, ue);
-    k2s_phase<R, false>(p, sm, threadIdx.x >> 5, threadIdx.x & 31, ub, ue, 0u);
+    k2s_phase<R, false, BX>(p, sm, threadIdx.x >> 5, threadIdx.x & 31, ub, ue, 0u);
 }

@@ -33,8 +33,9 @@
 #define K3_MAX_NW 11                                      // consumer warps (+1 producer warp)
 #endif
 #ifndef K3_RING
-#define K3_RING (176 / K3_SEG)                            // chunks in the ring (220 KB); must exceed 32 (see the producer)
+#define K3_RING (176 / K3_SEG)                            // chunks in the ring (220 KB)
 #endif
+#define K3_BATCH (K3_RING > 32 ? 32 : 16)                 // lanes of the producer warp that issue copies; must be < K3_RING (see the producer)
 
 template <int R> struct K3Geom {
     static constexpr int NIN = K3_SEG + 2 * R;           // input rows per task
@@ -173,7 +174,7 @@ template <int R> __device__ __forceinline__ int k3_cta_chunks(int t_begin, int t
 //   0: five planes in, nothing kept (default);  1: five planes in, a, b, c also stored to p.G (first iteration of a level);
 //   2: tmS is the two-plane map (box 64 x K3_SEG x 2) read at field 3: only IxIt, IyIt are fetched and summed, a, b, c come from p.G.
 // The value of every sum is formed by the same instructions in the same order in all three modes.
-template <int R, bool MK, int HM>
+template <int R, bool MK, int HM, bool BX>
 __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params &p, const K3Smem &sm, int warp, int lane, int nwc,
                                          int t_begin, int t_end, uint32_t gc0)
 {
@@ -199,11 +200,12 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             auto produce_run = [&](int s, int rb0, int ntask, int gbase) {
                 const int total = ntask + NC - 1;
                 const int x0 = 64 * s, yc0 = K3_SEG * rb0 - R;          // chunk c holds rows yc0 + K3_SEG*c ...
-                // batches of 32 chunks with a warp barrier in between: two uses of one ring slot are K3_RING > 32 chunks apart,
-                // so no lane can wait for a slot's release two uses ahead (an mbarrier only tells the parity of its phase)
-                for (int c0 = 0; c0 < total; c0 += 32) {
+                // batches of K3_BATCH chunks with a warp barrier in between: two uses of one ring slot are K3_RING > K3_BATCH chunks
+                // apart, so no lane can wait for a slot's release two uses ahead (an mbarrier only tells the parity of its phase)
+                static_assert(K3_RING > K3_BATCH && K3_RING >= NC + 2, "ring too small");
+                for (int c0 = 0; c0 < total; c0 += K3_BATCH) {
                     const int c = c0 + lane;
-                    if (c < total) {
+                    if (lane < K3_BATCH && c < total) {
                         const int gc = gbase + c, slot = gc % K3_RING, use = gc / K3_RING;
                         if (use > 0) mbar_wait(empty0 + 8 * slot, (use - 1) & 1);
                         const int readers = min(ntask - 1, c) - max(0, c - NC + 1) + 1;
@@ -305,7 +307,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
             for (int f = F0; f < 5; ++f) win_vfinish<K3_SEG, BOX>(acc[f], core[f]);
         };
         if (!OF_DBG(p.dbg, 2)) {
-            if (win_box_path(R) && p.ww.box) sum_rows(std::true_type()); else sum_rows(std::false_type());
+            sum_rows(std::integral_constant<bool, BX>());
         }
         __syncwarp();
         if (lane == 0 && !OF_DBG(p.dbg, 1)) {
@@ -331,7 +333,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
     }
 }
 
-template <int R, bool MK>
+template <int R, bool MK, bool BX>
 __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const __grid_constant__ CUtensorMap tmS, const K3Params p)
 {
     extern __shared__ __align__(1024) unsigned char k3_smem_[];
@@ -341,5 +343,5 @@ __global__ void __launch_bounds__(32 * (K3_MAX_NW + 1), 1) k3_vsum_solve(const _
     int t_begin, t_end;
     cta_range(p.ntasks, blockIdx.x, gridDim.x, t_begin, t_end);
     if (MK) { t_begin = p.md.k3_cta[blockIdx.x].ent_b; t_end = p.md.k3_cta[blockIdx.x].ent_e; }
-    k3_phase<R, MK, 0>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, t_begin, t_end, 0u);
+    k3_phase<R, MK, 0, BX>(&tmS, p, sm, threadIdx.x >> 5, threadIdx.x & 31, (blockDim.x >> 5) - 1, t_begin, t_end, 0u);
 }

@@ -35,6 +35,9 @@
 #ifndef SOLVE_WARPS
 #define SOLVE_WARPS 12                       // 11 K3 consumers + 1 producer; all 12 work in the K2 pass
 #endif
+#ifndef SOLVE_CTAS_PER_SM
+#define SOLVE_CTAS_PER_SM 1                  // 2 in the half-SM build (optflow_half.cu): two solves of different pairs share every SM
+#endif
 
 struct LevelDesc {
     const float *pyr[2];                     // pyramid slots (I1 / I2 chosen per job)
@@ -52,9 +55,13 @@ struct LevelDesc {
 // barriers and counters (720 B), then the K2 barriers, descriptors and ticket counter.
 #define SOLVE_K2S_BAR_OFF (K3_RING * K3_CHUNK_BYTES + 768)
 template <int R> struct SolveSmem {
+#if SOLVE_K2S
     static constexpr int BYTES = SOLVE_K2S_BAR_OFF + K2S<R>::BAR_BYTES;
     static_assert(K3Geom<R>::SMEM <= SOLVE_K2S_BAR_OFF && K2S<R>::DATA_BYTES <= K3_RING * K3_CHUNK_BYTES && K2S<R>::DATA_MAX == K3_RING * K3_CHUNK_BYTES,
                   "shared-memory map of the solve kernel");
+#else
+    static constexpr int BYTES = K3Geom<R>::SMEM;
+#endif
 };
 
 #define SOLVE_MAX_LEVELS 12
@@ -209,8 +216,9 @@ __device__ __forceinline__ void upsample_phase(const LevelDesc &F, const LevelDe
 // HO = of_set_hoist: IxIx, IxIy, IyIy and their window sums a, b, c are formed in the first iteration of a level only
 // (they depend on I1 alone, reading D9): later iterations write, fetch and sum the two It planes (60 B per pixel-iteration
 // instead of 72).  A separate instantiation: the default kernel carries none of it.
-template <int R, bool MK, bool HO>
-__global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __grid_constant__ SolveArgs a)
+// BX = box window: the sums take the add-only form (of_common.cuh).
+template <int R, bool MK, bool HO, bool BX>
+__global__ void __launch_bounds__(32 * SOLVE_WARPS, SOLVE_CTAS_PER_SM) of_solve_pair(const __grid_constant__ SolveArgs a)
 {
     extern __shared__ __align__(1024) unsigned char solve_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -253,7 +261,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
                 const FusedParams fp = {L.pyr[a.s1], L.pyr[a.s2], ui, vi, last ? a.u_out : uo, last ? a.v_out : vo, last ? a.valid : nullptr,
                                         last ? a.det : nullptr, L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.f_tw, L.f_th, L.f_tiles_x, L.f_ntiles,
                                         a.ww, a.sp, (l == top && it == 0) ? 1 : 0};
-                fused_iteration<R>(fp, solve_smem, cta, ncta);
+                fused_iteration<R, BX>(fp, solve_smem, cta, ncta);
                 prof_stamp(a, pi);                               // (four stamps per iteration, as in the two-pass form)
                 prof_stamp(a, pi);
                 prof_stamp(a, pi);
@@ -281,10 +289,10 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             p2.zero_uv = (l == top && it == 0) ? 1 : 0;            // zero initial guess at the coarsest level
             p2.f_first = (HO && it > 0) ? 3 : 0;
             if constexpr (MK || !SOLVE_K2S) {
-                k2_phase<R, MK, HO>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
+                k2_phase<R, MK, HO, BX>(p2, solve_smem, sm.counter + 1, warp, lane, k2_b, k2_e);
             } else {
                 q2.zero_uv = p2.zero_uv; q2.f_first = p2.f_first;
-                k2s_phase<R, HO>(q2, sm2, warp, lane, k2_b, k2_e, uk0);
+                k2s_phase<R, HO, BX>(q2, sm2, warp, lane, k2_b, k2_e, uk0);
                 uk0 += (uint32_t)(k2_e - k2_b);
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -296,9 +304,9 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_pair(const __gri
             K3Params p3 = {L.u, L.v, last ? a.u_out : L.u, last ? a.v_out : L.v, last ? a.valid : nullptr, last ? a.det : nullptr,
                            L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.k3_nrb, L.k3_ntasks, a.ww, a.sp, p2.zero_uv, a.dbg, M, HO ? a.G : nullptr, a.plane};
             if (warp == SOLVE_WARPS - 1 && lane == 0) asm volatile("fence.proxy.async.global;" ::: "memory");
-            if (!HO) k3_phase<R, MK, 0>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
-            else if (it == 0) k3_phase<R, MK, 1>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
-            else k3_phase<R, MK, 2>(&a.tm2[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            if (!HO) k3_phase<R, MK, 0, BX>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            else if (it == 0) k3_phase<R, MK, 1, BX>(&a.tm[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
+            else k3_phase<R, MK, 2, BX>(&a.tm2[l], p3, sm, warp, lane, SOLVE_WARPS - 1, k3_b, k3_e, gc0);
             gc0 += k3_chunks;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the ring was read by generic loads; the next K2 pass copies into it
             __syncthreads();

@@ -141,15 +141,15 @@ namespace {
 inline int round_up(int a, int b) { return (a + b - 1) / b * b; }
 inline unsigned long long k2s_magic(int nuy) { return ((1ull << 40) + (unsigned long long)nuy - 1) / (unsigned long long)nuy; }
 
-template <int R> int setup_attrs()
+template <int R, bool BX> int setup_attrs()
 {
 #if SOLVE_K2S
-    CU_TRY(cudaFuncSetAttribute(k2s_products_hsum<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k2s_products_hsum<R, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
 #else
-    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k2_products_hsum<R, false, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
 #endif
-    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
-    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(k3_vsum_solve<R, false, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    CU_TRY(cudaFuncSetAttribute(of_solve_pair<R, false, false, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
     return OF_OK;
 }
 
@@ -238,7 +238,7 @@ template <int R> void plan_level(of_context *c, int l)
     c->k2s_nunits[l] = ((c->lv[l].W + K2S<R>::TW - 1) / K2S<R>::TW) * c->k2s_nuy[l];
 }
 
-template <int R>
+template <int R, bool BX>
 void launch_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
 {
     const Level &L = c->lv[l];
@@ -248,15 +248,15 @@ void launch_k2(const of_context *c, int l, const float *I1, const float *I2, boo
                   c->ww, zero_uv ? 1 : 0, c->dbg, M.mask, M.k2_list, 0};
     if (M.mask) { of_launch_k2_masked(R, p, P.grid, 32 * P.warps, P.smem + 16, st); return; }    // compiled in optflow_mask.cu
 #if !SOLVE_K2S
-    k2_products_hsum<R, false><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
+    k2_products_hsum<R, false, BX><<<P.grid, 32 * P.warps, P.smem + 16, st>>>(p);
 #else
     const int s2 = I2 == c->pyr[1][l] ? 1 : 0;
     K2SParams q = {c->d_k2maps + l, s2, I1, I2, c->u[l], c->v[l], c->S, c->plane, L.W, L.H, L.pitch, c->k2s_nuy[l], c->k2s_nunits[l], k2s_magic(c->k2s_nuy[l]), c->ww, zero_uv ? 1 : 0, 0};
-    k2s_products_hsum<R><<<c->sms, 32 * (K2S_WORKERS + 1), K2S<R>::DATA_MAX + K2S<R>::BAR_BYTES, st>>>(q);
+    k2s_products_hsum<R, BX><<<c->sms, 32 * (K2S_WORKERS + 1), K2S<R>::DATA_MAX + K2S<R>::BAR_BYTES, st>>>(q);
 #endif
 }
 
-template <int R>
+template <int R, bool BX>
 void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st, uint8_t *valid_out = nullptr)
 {
     const Level &L = c->lv[l];
@@ -264,10 +264,10 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     K3Params p = {c->u[l], c->v[l], u_out, v_out, last ? (valid_out ? valid_out : c->valid) : nullptr, last ? c->det : nullptr,
                   L.W, L.H, L.pitch, out_pitch, P.nrb, P.ntasks, c->ww, {0.5f * c->eps_rel, c->max_step}, zero_uv ? 1 : 0, c->dbg, c->md[l], nullptr, 0};
     if (c->md[l].mask) of_launch_k3_masked(R, c->tmS[l], p, P.grid, 32 * (P.warps + 1), P.smem, st);
-    else k3_vsum_solve<R, false><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
+    else k3_vsum_solve<R, false, BX><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
-template <int R>
+template <int R, bool BX>
 cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int s2, float *u_out, float *v_out, cudaStream_t st, uint8_t *valid_out = nullptr)
 {
     static_assert(SOLVE_MAX_LEVELS == OF_MAX_LEVELS, "level limits out of sync");
@@ -283,7 +283,7 @@ cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int 
     void *args[] = {&a};
     if (ho) return of_launch_solve_hoisted(R, c->md[0].mask != nullptr, a, c->sms, st);     // compiled in optflow_hoist.cu
     if (c->md[0].mask) return of_launch_solve_masked(R, a, c->sms, st);                              // compiled in optflow_mask.cu
-    return cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, false, false>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
+    return cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, false, false, BX>, dim3(c->sms), dim3(32 * SOLVE_WARPS), args,
                                        (size_t)SolveSmem<R>::BYTES, st);
 }
 
@@ -349,11 +349,11 @@ int encode_tensor_maps(of_context *c)
 
 void run_k2(const of_context *c, int l, const float *I1, const float *I2, bool zero_uv, cudaStream_t st)
 {
-    DISPATCH_R(c->R, launch_k2<R>(c, l, I1, I2, zero_uv, st));
+    DISPATCH_RB(c->R, c->ww.box, (launch_k2<R, BX>(c, l, I1, I2, zero_uv, st)));
 }
 void run_k3(const of_context *c, int l, float *u_out, float *v_out, int out_pitch, bool last, bool zero_uv, cudaStream_t st, uint8_t *valid_out = nullptr)
 {
-    DISPATCH_R(c->R, launch_k3<R>(c, l, u_out, v_out, out_pitch, last, zero_uv, st, valid_out));
+    DISPATCH_RB(c->R, c->ww.box, (launch_k3<R, BX>(c, l, u_out, v_out, out_pitch, last, zero_uv, st, valid_out)));
 }
 
 void run_convert(const of_context *c, int dtype, const void *a, const void *b, float *da, float *db, cudaStream_t st)
@@ -449,7 +449,7 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
     const int top = c->levels - 1;     // (no memset of the coarsest field: its first iteration takes u = v = 0 without reading it)
     if (c->persistent) {
         cudaError_t e = cudaSuccess;
-        DISPATCH_R(c->R, e = launch_solve<R>(c, nullptr, j.s1, j.s2, j.u_out, j.v_out, st, j.valid_out));
+        DISPATCH_RB(c->R, c->ww.box, (e = launch_solve<R, BX>(c, nullptr, j.s1, j.s2, j.u_out, j.v_out, st, j.valid_out)));
         if (e != cudaSuccess && c->launch_err.empty()) c->launch_err = std::string("solve (persistent): ") + cudaGetErrorString(e);
         note_launch(c, "solve (persistent)", 0);
         return n + 1;
@@ -825,7 +825,7 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     }
     if (rc == OF_OK && cudaEventCreateWithFlags(&c->last_done, cudaEventDisableTiming) != cudaSuccess)
         rc = fail(OF_ERR_CUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
-    if (rc == OF_OK) { DISPATCH_R(window_radius, rc = setup_attrs<R>()); }
+    if (rc == OF_OK) { DISPATCH_RB(window_radius, c->ww.box, (rc = setup_attrs<R, BX>())); }
     if (rc == OF_OK) {
         cudaError_t e = of_setup_attrs_hoisted(window_radius, SMEM_MAX);
         if (e == cudaSuccess) e = of_setup_attrs_masked(window_radius, SMEM_MAX);
@@ -1062,7 +1062,7 @@ int of_run_solve(of_handle h, int repeat, void *stream)
     }
     for (int i = 0; i < repeat; ++i) {
         cudaError_t e = cudaSuccess;
-        DISPATCH_R(h->R, e = launch_solve<R>(h, nullptr, 0, 1, h->bench_out, h->bench_out + (size_t)h->W * h->H, st));
+        DISPATCH_RB(h->R, h->ww.box, (e = launch_solve<R, BX>(h, nullptr, 0, 1, h->bench_out, h->bench_out + (size_t)h->W * h->H, st)));
         if (e != cudaSuccess) return fail(OF_ERR_CUDA, "solve launch failed: %s", cudaGetErrorString(e));
     }
     return OF_OK;

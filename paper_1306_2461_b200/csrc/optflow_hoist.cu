@@ -9,7 +9,7 @@ cudaError_t of_launch_solve_hoisted(int R_, bool mk, const SolveArgs &a, int sms
     cudaError_t e = cudaErrorInvalidValue;
     SolveArgs args_copy = a;
     void *args[] = {&args_copy};
-    DISPATCH_R(R_, e = cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, false, true>, dim3(sms), dim3(32 * SOLVE_WARPS), args,
+    DISPATCH_RB(R_, a.ww.box, e = cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, false, true, BX>, dim3(sms), dim3(32 * SOLVE_WARPS), args,
                                                    (size_t)SolveSmem<R>::BYTES, st));
     return e;
 }
@@ -17,7 +17,10 @@ cudaError_t of_launch_solve_hoisted(int R_, bool mk, const SolveArgs &a, int sms
 cudaError_t of_setup_attrs_hoisted(int R_, int smem_max)
 {
     cudaError_t e = cudaErrorInvalidValue;
-    DISPATCH_R(R_, e = cudaFuncSetAttribute(of_solve_pair<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max));
+    for (int box = 0; box < 2; ++box) {
+        DISPATCH_RB(R_, box, e = cudaFuncSetAttribute(of_solve_pair<R, false, true, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max));
+        if (e != cudaSuccess) return e;
+    }
     if (e == cudaSuccess) e = of_setup_attrs_hoisted_masked(R_, smem_max);
     return e;
 }

@@ -4,12 +4,12 @@
 
 void of_launch_k2_masked(int R_, const K2Params &p, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    DISPATCH_R(R_, (k2_products_hsum<R, true><<<grid, threads, smem, st>>>(p)));
+    DISPATCH_RB(R_, p.ww.box, (k2_products_hsum<R, true, BX><<<grid, threads, smem, st>>>(p)));
 }
 
 void of_launch_k3_masked(int R_, const CUtensorMap &tm, const K3Params &p, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    DISPATCH_R(R_, (k3_vsum_solve<R, true><<<grid, threads, smem, st>>>(tm, p)));
+    DISPATCH_RB(R_, p.ww.box, (k3_vsum_solve<R, true, BX><<<grid, threads, smem, st>>>(tm, p)));
 }
 
 cudaError_t of_launch_solve_masked(int R_, const SolveArgs &a, int sms, cudaStream_t st)
@@ -17,7 +17,7 @@ cudaError_t of_launch_solve_masked(int R_, const SolveArgs &a, int sms, cudaStre
     cudaError_t e = cudaErrorInvalidValue;
     SolveArgs args_copy = a;
     void *args[] = {&args_copy};
-    DISPATCH_R(R_, e = cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, true, false>, dim3(sms), dim3(32 * SOLVE_WARPS), args,
+    DISPATCH_RB(R_, a.ww.box, e = cudaLaunchCooperativeKernel((const void *)of_solve_pair<R, true, false, BX>, dim3(sms), dim3(32 * SOLVE_WARPS), args,
                                                    (size_t)SolveSmem<R>::BYTES, st));
     return e;
 }
@@ -25,10 +25,13 @@ cudaError_t of_launch_solve_masked(int R_, const SolveArgs &a, int sms, cudaStre
 cudaError_t of_setup_attrs_masked(int R_, int smem_max)
 {
     cudaError_t e = cudaErrorInvalidValue;
-    DISPATCH_R(R_, {
-        e = cudaFuncSetAttribute(k2_products_hsum<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k3_vsum_solve<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(of_solve_pair<R, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
-    });
+    for (int box = 0; box < 2; ++box) {
+        DISPATCH_RB(R_, box, {
+            e = cudaFuncSetAttribute(k2_products_hsum<R, true, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(k3_vsum_solve<R, true, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(of_solve_pair<R, true, false, BX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+        });
+        if (e != cudaSuccess) return e;
+    }
     return e;
 }

@@ -26,6 +26,7 @@
 #ifndef OPTFLOW_H_
 #define OPTFLOW_H_
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -42,6 +43,8 @@ enum of_stream_mode { OF_STREAM_CONSECUTIVE = 0, OF_STREAM_PAIRS = 1 };
 #define OF_MAX_LEVELS 12
 #define OF_MAX_WINDOW_RADIUS 16
 #define OF_TIMELINE_MAX 4096
+#define OF_STATIC_MAX_PIXELS 16777216   /* of_field_minmax_static: largest field, 4096 x 4096 */
+#define OF_STATIC_SCRATCH_BYTES 33024   /* its static device array: 256 + 8 * OF_STATIC_MAX_PIXELS / 4096 */
 
 /* ---------------------------------------------------------------------------------------------
  * The three calls named by the north_star (BASELINE.json:5).
@@ -195,6 +198,20 @@ int of_bubble_count(of_handle h, const float *vx_dev, const uint8_t *valid_dev, 
 int of_bubble_threshold(of_handle h, const float *sum_dev, int n_fields, const uint8_t *valid_dev, float *threshold_dev, void *stream);
 int of_bubble_count_dev(of_handle h, const float *vx_dev, const uint8_t *valid_dev, const float *threshold_dev,
                         unsigned long long *out_dev, void *stream);
+/* of_field_minmax for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the same result -- out_dev[0] = min, out_dev[1] = max of field_dev[0..n) over the available vectors (valid_dev may
+ * be NULL), NaN ignored; the min / max step of eq. 3, PAPER.md:127-131 -- without a handle (of_create allocates) and without any
+ * cudaMalloc, cudaFree or allocating library routine.  All pointers are device pointers of the CURRENT device (field_dev, out_dev
+ * 4-byte aligned); asynchronous on `stream`; exact and bit-reproducible (integer min / max of per-chunk partials).
+ *   Scratch: one file-scope `static __device__` array of OF_STATIC_SCRATCH_BYTES (33 024) bytes in liboptflow.so, held by every
+ *   GPU that loads the library until the process exits.  It bounds the size: n > OF_STATIC_MAX_PIXELS (4096 x 4096) is rejected
+ *   with OF_ERR_INVALID_ARG and a message that names the limit (as are n == 0 and null / misaligned pointers).
+ *   Sharing: every call on a device uses the same array, which keeps the last call's contents; the call clears what must start
+ *   at zero itself.  Calls that may OVERLAP on the GPU (different streams with no ordering between them, concurrent host
+ *   threads) race on it and give wrong results: order them on one stream or with events.
+ *   The first call on each device looks up the array's device address (cudaGetSymbolAddress, no allocation); make that call once
+ *   before starting a graph capture. */
+int of_field_minmax_static(const float *field_dev, const uint8_t *valid_dev, size_t n, float *out_dev, void *stream);
 
 /* Stand-alone single steps (rows a2, a10 of the scope table), dense device buffers. */
 int of_pyramid_down(const float *src, int width, int height, float *dst, void *stream);

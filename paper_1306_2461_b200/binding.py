@@ -16,6 +16,7 @@ OF_WINDOW_BOX, OF_WINDOW_GAUSSIAN = 0, 1
 OF_DTYPE_F32, OF_DTYPE_U8, OF_DTYPE_U16 = 0, 1, 2
 OF_STREAM_CONSECUTIVE, OF_STREAM_PAIRS = 0, 1
 OF_OK = 0
+OF_STATIC_MAX_PIXELS = 16777216
 OF_ERR_INVALID_ARG, OF_ERR_ALLOC, OF_ERR_CUDA, OF_ERR_STATE = -1, -2, -3, -4
 
 _c = ctypes
@@ -49,6 +50,7 @@ SIGNATURES = {
     "of_field_accumulate": (_i, [_vp, _vp, _vp, _vp]),
     "of_field_minmax": (_i, [_vp, _vp, _vp, _vp, _vp]),
     "of_bubble_count": (_i, [_vp, _vp, _vp, _c.c_float, _vp, _vp]),
+    "of_field_minmax_static": (_i, [_vp, _vp, _c.c_size_t, _vp, _vp]),
     "of_pyramid_down": (_i, [_vp, _i, _i, _vp, _vp]),
     "of_upsample_flow": (_i, [_vp, _vp, _i, _i, _vp, _vp, _i, _i, _vp]),
     "of_stream_open": (_i, [_vp, _i, _i, _i]),
@@ -95,6 +97,14 @@ def _stream_ptr(stream=None):
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     return _vp(s.cuda_stream)
+
+
+def field_minmax_static(field, out, valid=None, stream=None):
+    """of_field_minmax_static: min / max of `field` over the available vectors into the caller's `out` (2 floats, device).
+    No handle and no allocation (static device scratch; at most OF_STATIC_MAX_PIXELS elements; calls must not overlap on the GPU)."""
+    _check(lib().of_field_minmax_static(field.data_ptr(), valid.data_ptr() if valid is not None else None,
+                                        field.numel(), out.data_ptr(), _stream_ptr(stream)))
+    return out
 
 
 class OpticalFlow:

@@ -8,8 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liboptflow.so")
-SOURCES = ["optflow.cu", "optflow_hoist.cu", "optflow_hoist_mask.cu", "optflow_mask.cu"]     # compiled in parallel (one nvcc process each), then linked
-DEPS = ["optflow.cu", "optflow_hoist.cu", "optflow_hoist_mask.cu", "optflow_mask.cu", "of_dispatch.cuh", "of_kernels.cuh", "of_common.cuh", "of_k2.cuh", "of_k2s.cuh", "of_async.cuh", "of_fused.cuh", "of_k3.cuh", "of_solve.cuh", "of_equalise.cuh", "of_post.cuh", os.path.join("..", "..", "include", "optflow.h")]
+SOURCES = ["optflow.cu", "optflow_hoist.cu", "optflow_hoist_mask.cu", "optflow_mask.cu", "optflow_static.cu"]     # compiled in parallel (one nvcc process each), then linked
+DEPS = ["optflow.cu", "optflow_hoist.cu", "optflow_hoist_mask.cu", "optflow_mask.cu", "optflow_static.cu", "of_dispatch.cuh", "of_kernels.cuh", "of_common.cuh", "of_k2.cuh", "of_k2s.cuh", "of_async.cuh", "of_fused.cuh", "of_k3.cuh", "of_solve.cuh", "of_equalise.cuh", "of_post.cuh", os.path.join("..", "..", "include", "optflow.h")]
 # OF_NVCC_DEFS="--split-compile 8" cuts the build from ~140 s to ~50 s, but nvcc then picks a different register allocation from
 # run to run (measured: 156/160, 162/156 or 166/168 registers for the two R = 12 solve kernels), so it is not the default:
 # the library that is tested must be the library that is rebuilt from the same sources.

@@ -744,6 +744,9 @@ void pipe_release(of_context *c)
 
 }  // namespace
 
+// error reporting for the other translation units (optflow_static.cu): sets the string of_last_error returns
+int of_detail_fail(int code, const char *msg) { return fail(code, "%s", msg); }
+
 // =================================================================================================
 // C ABI
 // =================================================================================================

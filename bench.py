@@ -246,6 +246,12 @@ def run_ours(args):
     d_out = [(torch.empty((H, W), dtype=torch.float32, device=dev), torch.empty((H, W), dtype=torch.float32, device=dev))
              for _ in range(nring)]
     of = B.OpticalFlow(*c0.create_args)
+    if args.mask != "none":                                     # obstacle mask (row f4): masked tiles and tasks are skipped
+        from paper_1306_2461_b200 import synthetic as syn
+        m = syn.mask_backward_step(W, H) if args.mask == "step" else np.ones((H, W), np.uint8)
+        if args.mask == "half":
+            m[:, W // 2:] = 0
+        of.set_mask(m)
     stream = torch.cuda.Stream(device=dev)
 
     def barrier():
@@ -287,6 +293,45 @@ def run_ours(args):
         of.compute(d_in[0][0], d_in[0][1], d_out[0][0], d_out[0][1])
     stream.synchronize()
     tl = of.solve_timeline(False).astype(np.float64)
+
+    # ---------------- throughput mode: two pairs per launch (of_compute_dual: the passes of two independent pairs alternate in one
+    # persistent kernel and the grid barrier of one pair is waited for behind a pass of the other; results bit-identical to of_compute)
+    dual = None
+    if not args.no_dual and nring >= 2 and args.mask == "none":      # (a masked handle cannot share a launch: of_compute_dual would fall back)
+        of2 = B.OpticalFlow(*c0.create_args)
+        npair2 = nring // 2
+
+        def dual_step(k):
+            i, j = 2 * (k % npair2), 2 * (k % npair2) + 1
+            B.compute_dual(of, of2, d_in[i][0], d_in[i][1], d_in[j][0], d_in[j][1], d_out[i][0], d_out[i][1], d_out[j][0], d_out[j][1])
+        with torch.cuda.stream(stream):
+            for k in range(max(args.warmup, 3) + npair2):
+                dual_step(k)
+        barrier()
+        nd = max(1, args.steps // 2)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            g0.record()
+            for k in range(nd):
+                dual_step(k)
+            g1.record()
+        barrier()
+        d_ms = reduce_max_time(g0.elapsed_time(g1), dist, dev)
+        d_launches = of.last_launch_count() * nd
+        with torch.cuda.stream(stream):
+            B.run_solve_dual(of, of2, 5)
+            g0.record()
+            B.run_solve_dual(of, of2, 100)
+            g1.record()
+            g1.synchronize()
+            d_solve_us = g0.elapsed_time(g1) / 100 * 1e3
+        of.solve_timeline(True)
+        with torch.cuda.stream(stream):
+            dual_step(0)
+        stream.synchronize()
+        d_tl = of.solve_timeline(False).astype(np.float64)
+        dual = (d_ms, 2 * nd, d_launches, d_solve_us, d_tl)
+        of2.close()
 
     # ---------------- the same job with of_set_hoist(1) (opt-in; bit-identical results; reported beside the headline, which
     # stays the five-plane form BASELINE.json's north_star states)
@@ -405,30 +450,72 @@ def run_ours(args):
         px = W * H
         level_px = [((W + (1 << l) - 1) >> l) * ((H + (1 << l) - 1) >> l) for l in range(c0.levels)]
         pix_iters = sum(level_px) * c0.iterations
-        solve_bytes = 72.0 * pix_iters
-        ach = solve_bytes / (solve_us * 1e-6) / 1e9
-        # level-0 iteration from the in-kernel timeline: {K2 pass, barrier, K3 pass, barrier} medians
         mhz = clocks.get("sm_mhz") or 1965.0
         L, it = c0.levels, c0.iterations
-        d = np.diff(tl) / mhz                                  # us per phase
         i0 = 2 * (L - 1) + 4 * it * (L - 1)                    # first phase of level 0's iterations
-        seg = d[i0:i0 + 4 * it].reshape(it, 4)
-        med = np.median(seg[:-1], axis=0) if it > 1 else seg[0]
-        iter_us = float(med.sum())
-        iter_gbs = 72.0 * px / (iter_us * 1e-6) / 1e9
-        value = world * args.steps / (ms * 1e-3)
-        # every level, coarse to fine (a fused coarse level has one pass and one barrier per iteration: its time is under k2_pass)
-        levels_tl, k = [], 0
-        for l in range(L - 1, -1, -1):
-            if l < L - 1:
-                levels_tl.append({"level": l, "hand_down_us": float(d[k]), "hand_down_barrier_us": float(d[k + 1])})
-                k += 2
-            sg = d[k:k + 4 * it].reshape(it, 4)
-            k += 4 * it
-            m4 = np.median(sg[:-1], axis=0) if it > 1 else sg[0]
-            levels_tl.append({"level": l, "pixels": level_px[l], "k2_pass_us": float(m4[0]), "barrier_1_us": float(m4[1]), "k3_pass_us": float(m4[2]),
-                              "barrier_2_us": float(m4[3]), "iteration_us": float(m4.sum()),
-                              "frac_of_peak": 72.0 * level_px[l] / (float(m4.sum()) * 1e-6) / 1e9 / peak})
+        traffic, traffic_src = ncu_dram_bytes(args.workload)
+
+        def analyse(tl_, solve_us_, npairs, kernel):
+            """Roofline of the solve kernel and per-level timeline from the in-kernel stamps; npairs = pairs one launch solves."""
+            solve_bytes = 72.0 * pix_iters * npairs
+            ach = solve_bytes / (solve_us_ * 1e-6) / 1e9
+            d = np.diff(tl_) / mhz                              # us per phase
+            # level-0 iteration: {K2 pass, barrier, K3 pass, barrier} medians over the iterations
+            seg = d[i0:i0 + 4 * it].reshape(it, 4)
+            med = np.median(seg[:-1], axis=0) if it > 1 else seg[0]
+            iter_us = float(med.sum())
+            iter_gbs = 72.0 * px * npairs / (iter_us * 1e-6) / 1e9
+            # every level, coarse to fine (a fused coarse level has one pass and one barrier per iteration: its time is under k2_pass)
+            levels_tl, k = [], 0
+            for l in range(L - 1, -1, -1):
+                if l < L - 1:
+                    levels_tl.append({"level": l, "hand_down_us": float(d[k]), "hand_down_barrier_us": float(d[k + 1])})
+                    k += 2
+                sg = d[k:k + 4 * it].reshape(it, 4)
+                k += 4 * it
+                m4 = np.median(sg[:-1], axis=0) if it > 1 else sg[0]
+                levels_tl.append({"level": l, "pixels": level_px[l], "k2_pass_us": float(m4[0]), "barrier_1_us": float(m4[1]), "k3_pass_us": float(m4[2]),
+                                  "barrier_2_us": float(m4[3]), "iteration_us": float(m4.sum()),
+                                  "frac_of_peak": 72.0 * level_px[l] * npairs / (float(m4.sum()) * 1e-6) / 1e9 / peak})
+            roof = {"bound": "hbm", "kernel": kernel, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": traffic * npairs if traffic is not None else None, "traffic_source": traffic_src,
+                    "peak_source": peak_src, "bytes_per_launch": solve_bytes,
+                    "bytes_basis": "72 B per pixel-iteration (K2 16 R + 20 W, K3 28 R + 8 W; SURVEY.md 8(d)) x %d pixel-iterations x %d pair(s) per launch"
+                                   % (pix_iters, npairs),
+                    "us_per_launch": solve_us_,
+                    "note": "algorithmic bytes over time against the HBM copy peak, as SURVEY.md 8(d) defines the bar; at 1280x1024 the planes are "
+                            "L2 resident (see traffic: the single-pair capture x pairs per launch), so the limiter is latency / issue rate, not DRAM: "
+                            "against the measured L2-resident streaming rate of the same byte mix the fraction is frac_of_l2_streaming",
+                    "frac_of_l2_streaming": ach / L2_STREAM_GBPS, "l2_streaming_GBps": L2_STREAM_GBPS}
+            it0 = {"bytes": 72 * px * npairs, "us": iter_us, "GB/s": iter_gbs, "frac_of_peak": iter_gbs / peak,
+                   "phases_us": {"k2_pass": float(med[0]), "barrier_1": float(med[1]), "k3_pass": float(med[2]), "barrier_2": float(med[3])},
+                   "how": "in-kernel SM cycle stamps (of_solve_timeline, max over CTAs) / sampled SM clock; median over iterations" +
+                          ("; one iteration of BOTH pairs (K2 pass of a, of b, K3 pass of a, of b; the barriers are waited for behind the other pair's pass)"
+                           if npairs == 2 else "")}
+            return roof, it0, levels_tl
+
+        s_value = world * args.steps / (ms * 1e-3)
+        s_roof, s_it0, s_levels = analyse(tl, solve_us, 1, "of_solve_pair<R, false, false> (persistent: K2 pass + K3 pass per iteration, fused coarse "
+                                                          "levels, hand-down; all levels and iterations of one pair)")
+        single = {"api": "of_compute (one pair per launch: lowest latency)", "value": s_value, "unit": UNIT, "ms_per_step": ms / args.steps,
+                  "gpu_launches": launches, "roofline": s_roof, "iteration_level0": s_it0, "levels_timeline": s_levels}
+        # the headline is the faster of the two launch modes of the public API; the other one is reported beside it
+        dual_out = None
+        if dual is not None:
+            d_ms, d_pairs, d_launches, d_solve_us, d_tl = dual
+            d_roof, d_it0, d_levels = analyse(d_tl, d_solve_us, 2, "of_solve_dual<R> (persistent, two pairs per launch: the passes of the two pairs alternate, "
+                                                                  "split grid barriers; K2 pass + K3 pass per iteration, fused coarse levels, hand-down)")
+            dual_out = {"api": "of_compute_dual (two pairs of two handles per launch: throughput mode; results bit-identical to of_compute)",
+                        "value": world * d_pairs / (d_ms * 1e-3), "unit": UNIT, "ms_per_step": d_ms / d_pairs, "steps": d_pairs,
+                        "gpu_launches": d_launches, "roofline": d_roof, "iteration_level0": d_it0, "levels_timeline": d_levels}
+        if dual_out is not None and dual_out["value"] > s_value:
+            value, ms_per_step, n_launch, steps_timed = dual_out["value"], dual_out["ms_per_step"], dual_out["gpu_launches"], dual_out["steps"]
+            roof, it0, levels_tl = dual_out["roofline"], dual_out["iteration_level0"], dual_out["levels_timeline"]
+            launch_mode = "two pairs per launch (of_compute_dual): the faster mode on this workload; one pair per launch under single_pair"
+        else:
+            value, ms_per_step, n_launch, steps_timed = s_value, ms / args.steps, launches, args.steps
+            roof, it0, levels_tl = s_roof, s_it0, s_levels
+            launch_mode = "one pair per launch (of_compute)" + ("" if dual_out is None else ": the faster mode on this workload; two pairs per launch under dual_launch")
         hoist_out = None
         if hoist is not None:
             h_ms, h_solve_us, h_tl = hoist
@@ -440,7 +527,7 @@ def run_ours(args):
             h_bytes = (84.0 + 60.0 * (it - 1)) * sum(level_px)
             hoist_out = {"api": "of_set_hoist(handle, 1): IxIx, IxIy, IyIy and their window sums formed in the first iteration of a "
                                 "level only (SURVEY.md 8(f) note f5); results bit-identical to the headline run "
-                                "(tests/test_gpu_parity.py::test_hoisted_invariant_planes_agree_bitwise); opt-in",
+                                "(tests/test_gpu_parity.py::test_hoisted_invariant_planes_agree_bitwise); opt-in; one pair per launch",
                          "value": world * args.steps / (h_ms * 1e-3), "unit": UNIT, "ms_per_step": h_ms / args.steps,
                          "kernel": "of_solve_pair<R, false, true>", "us_per_launch": h_solve_us,
                          "bytes_per_launch": h_bytes, "achieved_GB/s": h_bytes / (h_solve_us * 1e-6) / 1e9,
@@ -449,35 +536,26 @@ def run_ours(args):
                                               "frac_of_peak": 60.0 * px / (h_iter_us * 1e-6) / 1e9 / peak,
                                               "phases_us": {"k2_pass": float(hmed[0]), "barrier_1": float(hmed[1]),
                                                             "k3_pass": float(hmed[2]), "barrier_2": float(hmed[3])}}}
-        traffic, traffic_src = ncu_dram_bytes(args.workload)
         planes_mb = 9 * 4 * px / 1e6
         out = {
-            "metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps_timed, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl, "levels": c0.levels, "window_radius": c0.window_radius, "iterations": c0.iterations,
                        "window": "gaussian" if c0.window_type == B.OF_WINDOW_GAUSSIAN else "box", "parallelism": "replicas only x%d" % world,
+                       "launch": launch_mode, "mask": args.mask,
                        "l2": "inputs and outputs rotate over a ring of %d pairs (%.0f MB; L2 is 126 MB); the %.0f MB of internal planes of the "
                              "finest level %s" % (nring, nring * (2 * px * esize + 8 * px) / 1e6, planes_mb,
                                                   "exceed L2: this workload is HBM bound" if planes_mb > 126 else "are L2 resident at this size")},
             "mpixel_iterations_per_s": value * pix_iters / 1e6,
             "clocks": clocks,
             "e2e": e2e,
-            "gpu_launches": launches,
-            "roofline": {"bound": "hbm", "kernel": "of_solve_pair<R, false, false> (persistent: K2 pass + K3 pass per iteration, fused coarse levels, hand-down; all levels and iterations)",
-                         "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                         "traffic": traffic, "traffic_source": traffic_src,
-                         "peak_source": peak_src, "bytes_per_launch": solve_bytes,
-                         "bytes_basis": "72 B per pixel-iteration (K2 16 R + 20 W, K3 28 R + 8 W; SURVEY.md 8(d)) x %d pixel-iterations" % pix_iters,
-                         "us_per_launch": solve_us,
-                         "note": "algorithmic bytes over time against the HBM copy peak, as SURVEY.md 8(d) defines the bar; at this size the planes are "
-                                 "L2 resident (see traffic), so the limiter is latency / issue rate, not DRAM: against the measured L2-resident "
-                                 "streaming rate of the same byte mix the fraction is frac_of_l2_streaming",
-                         "frac_of_l2_streaming": ach / L2_STREAM_GBPS, "l2_streaming_GBps": L2_STREAM_GBPS},
-            "iteration_level0": {"bytes": 72 * px, "us": iter_us, "GB/s": iter_gbs, "frac_of_peak": iter_gbs / peak,
-                                 "phases_us": {"k2_pass": float(med[0]), "barrier_1": float(med[1]), "k3_pass": float(med[2]), "barrier_2": float(med[3])},
-                                 "how": "in-kernel SM cycle stamps (of_solve_timeline, max over CTAs) / sampled SM clock; median over iterations"},
+            "gpu_launches": n_launch,
+            "roofline": roof,
+            "iteration_level0": it0,
             "levels_timeline": levels_tl,
+            "single_pair": single if (dual_out is not None and dual_out["value"] > s_value) else None,
+            "dual_launch": dual_out if not (dual_out is not None and dual_out["value"] > s_value) else None,
             "variant_hoist": hoist_out,
             "cpu_baseline": cpu,
             "cpu_baseline_1thread": cpu1,
@@ -499,6 +577,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer pipeline leg (profiling runs)")
     ap.add_argument("--no-hoist", action="store_true", help="skip the of_set_hoist(1) variant leg (profiling runs)")
+    ap.add_argument("--no-dual", action="store_true", help="skip the two-pairs-per-launch leg (of_compute_dual); the headline is then the single-pair launch")
+    ap.add_argument("--mask", default="none", choices=["none", "step", "half"],
+                    help="obstacle mask set on the handle (of_set_mask): step = synthetic.mask_backward_step (14 %% obstacle), half = right half of the frame")
     ap.add_argument("--ring", type=int, default=RING, help="distinct input pairs / output buffers cycled through")
     args = ap.parse_args()
     if args.impl == "reference":

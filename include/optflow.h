@@ -82,6 +82,21 @@ void of_destroy(of_handle h);
 int of_compute_u8(of_handle h, const uint8_t *I1, const uint8_t *I2, float *u, float *v, void *stream);
 int of_compute_u16(of_handle h, const uint16_t *I1, const uint16_t *I2, float *u, float *v, void *stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Throughput mode: TWO independent pairs in one launch ("the computation of a velocity field is independent of all
+ * other computations"; the stream of image pairs).  Pair a is solved with handle ha, pair b with handle hb --
+ * two different handles created with the same arguments on the same device, each providing the scratch of its pair -- exactly as
+ * of_compute / of_compute_u8 / of_compute_u16 would solve them (dtype = an of_dtype value for all four frames; same pointer rules;
+ * both results are bit-identical to the single calls), but by one persistent kernel in which the passes of the two pairs alternate
+ * and the grid-wide barrier of one pair is waited for behind a pass of the other (csrc/of_solve_dual.cuh).  What it buys is pairs
+ * per second; what it costs is latency: neither field is complete before the launch ends.  Enqueue only, no allocation; both
+ * handles count as busy until it ends (a later call on either is ordered after it).  If the handles cannot share a launch (different
+ * sizes, parameters or conditioning, a mask, of_set_hoist(1) or of_set_persistent(0) on either), the two pairs are solved one after the other by
+ * two ordinary solves, with the same results.  The validity mask of each pair is its handle's (of_get_validity).
+ * ------------------------------------------------------------------------------------------- */
+int of_compute_dual(of_handle ha, of_handle hb, int dtype, const void *I1a, const void *I2a, float *ua, float *va,
+                    const void *I1b, const void *I2b, float *ub, float *vb, void *stream);
+
 /* Text of the calling thread's last error ("" if none).  Never NULL. */
 const char *of_last_error(void);
 
@@ -165,6 +180,10 @@ int of_run_step(of_handle h, int level, int which, int repeat, void *stream);
  * on the pyramids left by the last of_compute*; the level-0 result is discarded into scratch.  For
  * timing the dominant kernel with CUDA events and for ncu. */
 int of_run_solve(of_handle h, int repeat, void *stream);
+/* The same for the two-pair kernel of of_compute_dual (pyramids left by the last solves of ha and hb); fails with OF_ERR_STATE
+ * if the handles cannot share a launch.  With the timeline hook on for ha, of_solve_timeline(ha) returns the stamps of that kernel:
+ * same positions as for one pair, each pass interval covering the pass of both pairs (the barrier intervals are empty). */
+int of_run_solve_dual(of_handle ha, of_handle hb, int repeat, void *stream);
 
 /* Timeline of the persistent solve kernel (profiling hook; the in-kernel analogue of a launch list).
  * While the hook is on, thread 0 of every CTA stores its SM cycle counter, relative to the CTA's start,

@@ -29,6 +29,8 @@ SIGNATURES = {
     "of_destroy": (None, [_vp]),
     "of_compute_u8": (_i, [_vp] * 6),
     "of_compute_u16": (_i, [_vp] * 6),
+    "of_compute_dual": (_i, [_vp, _vp, _i] + [_vp] * 9),
+    "of_run_solve_dual": (_i, [_vp, _vp, _i, _vp]),
     "of_last_error": (_c.c_char_p, []),
     "of_set_conditioning": (_i, [_vp, _c.c_float, _c.c_float]),
     "of_set_equalisation": (_i, [_vp, _i]),
@@ -105,6 +107,39 @@ def field_minmax_static(field, out, valid=None, stream=None):
     _check(lib().of_field_minmax_static(field.data_ptr(), valid.data_ptr() if valid is not None else None,
                                         field.numel(), out.data_ptr(), _stream_ptr(stream)))
     return out
+
+
+def _dtype_code(t, torch):
+    if t == torch.float32:
+        return OF_DTYPE_F32
+    if t == torch.uint8:
+        return OF_DTYPE_U8
+    if t in (torch.uint16, torch.int16):
+        return OF_DTYPE_U16
+    raise OptflowError("unsupported image dtype %s" % t)
+
+
+def compute_dual(ofa, ofb, I1a, I2a, I1b, I2b, ua=None, va=None, ub=None, vb=None, stream=None):
+    """of_compute_dual: pair a with handle `ofa`, pair b with handle `ofb` (two OpticalFlow objects created with the same
+    arguments), one launch for both (throughput mode).  Returns (ua, va, ub, vb); same tensors rules as OpticalFlow.compute."""
+    import torch
+    H, W = ofa.height, ofa.width
+    outs = []
+    for f in (ua, va, ub, vb):
+        if f is None:
+            f = torch.empty((H, W), dtype=torch.float32, device=I1a.device)
+        assert f.is_cuda and f.is_contiguous() and f.dtype == torch.float32 and tuple(f.shape) == (H, W)
+        outs.append(f)
+    for t in (I1a, I2a, I1b, I2b):
+        assert t.is_cuda and t.is_contiguous() and tuple(t.shape) == (H, W) and t.dtype == I1a.dtype
+    _check(lib().of_compute_dual(ofa._h, ofb._h, _dtype_code(I1a.dtype, torch), I1a.data_ptr(), I2a.data_ptr(), outs[0].data_ptr(),
+                                 outs[1].data_ptr(), I1b.data_ptr(), I2b.data_ptr(), outs[2].data_ptr(), outs[3].data_ptr(),
+                                 _stream_ptr(stream)))
+    return tuple(outs)
+
+
+def run_solve_dual(ofa, ofb, repeat=1, stream=None):
+    _check(lib().of_run_solve_dual(ofa._h, ofb._h, repeat, _stream_ptr(stream)))
 
 
 class OpticalFlow:

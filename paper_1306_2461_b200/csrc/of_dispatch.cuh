@@ -44,3 +44,7 @@ void of_launch_k2_masked(int R, const K2Params &p, int grid, int threads, size_t
 void of_launch_k3_masked(int R, const CUtensorMap &tm, const K3Params &p, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t of_launch_solve_masked(int R, const SolveArgs &a, int sms, cudaStream_t st);
 cudaError_t of_setup_attrs_masked(int R, int smem_max);
+
+// optflow_dual.cu: of_solve_dual<R, BX> (of_solve_dual.cuh), two pairs of two handles in one cooperative launch (unmasked, un-hoisted).
+cudaError_t of_launch_solve_dual(int R, const SolveArgs &a0, const SolveArgs &a1, int sms, cudaStream_t st);
+cudaError_t of_setup_attrs_dual(int R, int smem_max);

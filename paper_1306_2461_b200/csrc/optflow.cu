@@ -267,19 +267,25 @@ void launch_k3(const of_context *c, int l, float *u_out, float *v_out, int out_p
     else k3_vsum_solve<R, false, BX><<<P.grid, 32 * (P.warps + 1), P.smem, st>>>(c->tmS[l], p);
 }
 
-template <int R, bool BX>
-cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int s2, float *u_out, float *v_out, cudaStream_t st, uint8_t *valid_out = nullptr)
+// Arguments of the persistent solve kernel for one pair of handle c (of_solve_pair, of_solve_dual).
+void fill_solve_args(const of_context *c, int s1, int s2, float *u_out, float *v_out, uint8_t *valid_out, SolveArgs &a)
 {
     static_assert(SOLVE_MAX_LEVELS == OF_MAX_LEVELS, "level limits out of sync");
-    SolveArgs a;
     memcpy(a.tm, c->tmS, sizeof(CUtensorMap) * c->levels);
     a.lv = c->d_lv; a.gbar = c->d_gbar; a.S = c->S; a.plane = c->plane; a.u_out = u_out; a.v_out = v_out;
     a.valid = valid_out ? valid_out : c->valid; a.det = c->det; a.levels = c->levels; a.iterations = c->iterations; a.s1 = s1; a.s2 = s2;
     a.md = c->d_md; a.G = c->G; a.k2maps = c->d_k2maps;
-    const bool ho = c->hoist && c->G != nullptr;
-    if (ho) memcpy(a.tm2, c->tmS2, sizeof(CUtensorMap) * c->levels);
+    if (c->hoist && c->G != nullptr) memcpy(a.tm2, c->tmS2, sizeof(CUtensorMap) * c->levels);
     a.out_pitch = c->W; a.dbg = c->dbg; a.prof = c->prof_on ? c->d_prof : nullptr; a.ww = c->ww;
     a.sp.eps_half = 0.5f * c->eps_rel; a.sp.max_step = c->max_step;
+}
+
+template <int R, bool BX>
+cudaError_t launch_solve(const of_context *c, const float *const *, int s1, int s2, float *u_out, float *v_out, cudaStream_t st, uint8_t *valid_out = nullptr)
+{
+    SolveArgs a;
+    fill_solve_args(c, s1, s2, u_out, v_out, valid_out, a);
+    const bool ho = c->hoist && c->G != nullptr;
     void *args[] = {&a};
     if (ho) return of_launch_solve_hoisted(R, c->md[0].mask != nullptr, a, c->sms, st);     // compiled in optflow_hoist.cu
     if (c->md[0].mask) return of_launch_solve_masked(R, a, c->sms, st);                              // compiled in optflow_mask.cu
@@ -420,8 +426,8 @@ void note_launch(of_context *c, const char *what, int level)
     }
 }
 
-// Enqueue the whole path of one Job (rows a1-a10).  Returns the number of kernels launched.
-int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
+// Frame conversion + pyramid of one Job (rows a1-a2).  Returns the number of kernels launched.
+int enqueue_pyramids(of_context *c, const Job &j, cudaStream_t st)
 {
     int n = 0;
     c->launch_err.clear();
@@ -446,6 +452,13 @@ int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
             ++n;
         }
     }
+    return n;
+}
+
+// Enqueue the whole path of one Job (rows a1-a10).  Returns the number of kernels launched.
+int enqueue_job(of_context *c, const Job &j, cudaStream_t st)
+{
+    int n = enqueue_pyramids(c, j, st);
     const int top = c->levels - 1;     // (no memset of the coarsest field: its first iteration takes u = v = 0 without reading it)
     if (c->persistent) {
         cudaError_t e = cudaSuccess;
@@ -695,20 +708,63 @@ int dev_alloc(of_context *c, void **p, size_t bytes)
     return OF_OK;
 }
 
-int compute_any(of_handle h, int dtype, const void *I1, const void *I2, float *u, float *v, void *stream)
+// Argument checks of one pair and its Job.
+int make_pair_job(of_handle h, int dtype, const void *I1, const void *I2, float *u, float *v, Job &j)
 {
     if (!h) return fail(OF_ERR_INVALID_ARG, "null handle");
     if (!I1 || !I2 || !u || !v) return fail(OF_ERR_INVALID_ARG, "null image or field pointer");
     if (h->pipe.open) return fail(OF_ERR_STATE, "handle is in streaming mode; call of_stream_close first");
     if ((reinterpret_cast<uintptr_t>(u) | reinterpret_cast<uintptr_t>(v)) & 15)
         return fail(OF_ERR_INVALID_ARG, "u and v must be 16-byte aligned (the last pass stores float2 / float4)");
+    if (dtype != OF_DTYPE_F32 && dtype != OF_DTYPE_U8 && dtype != OF_DTYPE_U16) return fail(OF_ERR_INVALID_ARG, "unknown dtype %d", dtype);
     const size_t es = dtype == OF_DTYPE_U8 ? 1 : (dtype == OF_DTYPE_U16 ? 2 : 4);
     if ((reinterpret_cast<uintptr_t>(I1) | reinterpret_cast<uintptr_t>(I2)) & (es - 1))
         return fail(OF_ERR_INVALID_ARG, "I1 and I2 must be aligned to their element size");
-    Job j;
     memset(&j, 0, sizeof j);
     j.dtype = dtype; j.rawA = I1; j.rawB = I2; j.cvtA = 0; j.cvtB = 1; j.s1 = 0; j.s2 = 1; j.u_out = u; j.v_out = v;
+    return OF_OK;
+}
+
+int compute_any(of_handle h, int dtype, const void *I1, const void *I2, float *u, float *v, void *stream)
+{
+    Job j;
+    int rc = make_pair_job(h, dtype, I1, I2, u, v, j);
+    if (rc != OF_OK) return rc;
     return submit_job(h, j, (cudaStream_t)stream);
+}
+
+// Two handles can share one of_solve_dual launch iff they describe the same problem and neither needs a variant kernel.
+bool dual_eligible(const of_context *a, const of_context *b)
+{
+    return a != b && a->device == b->device && a->W == b->W && a->H == b->H && a->levels == b->levels && a->R == b->R &&
+           a->iterations == b->iterations && a->window_type == b->window_type && a->persistent && b->persistent &&
+           a->fuse_coarse == b->fuse_coarse && a->eps_rel == b->eps_rel && a->max_step == b->max_step && !a->md[0].mask && !b->md[0].mask && !(a->hoist && a->G) && !(b->hoist && b->G) &&
+           a->dbg == 0 && b->dbg == 0;
+}
+
+// Both pairs: conversion + pyramids of each, then ONE solve launch for the two (of_solve_dual.cuh).  Both handles are busy until it ends.
+int submit_dual(of_context *a, const Job &ja, of_context *b, const Job &jb, cudaStream_t st)
+{
+    CU_TRY(cudaSetDevice(a->device));
+    if (a->have_last && st != a->last_stream) CU_TRY(cudaStreamWaitEvent(st, a->last_done, 0));
+    if (b->have_last && st != b->last_stream) CU_TRY(cudaStreamWaitEvent(st, b->last_done, 0));
+    int n = enqueue_pyramids(a, ja, st);
+    n += enqueue_pyramids(b, jb, st);
+    SolveArgs sa, sb;
+    fill_solve_args(a, ja.s1, ja.s2, ja.u_out, ja.v_out, ja.valid_out, sa);
+    fill_solve_args(b, jb.s1, jb.s2, jb.u_out, jb.v_out, jb.valid_out, sb);
+    sb.prof = nullptr;                                     // the timeline of a two-pair launch is kept by the first handle
+    cudaError_t e = of_launch_solve_dual(a->R, sa, sb, a->sms, st);
+    if (e != cudaSuccess) return fail(OF_ERR_CUDA, "solve (two pairs) launch failed: %s; first failing launch before it: %s", cudaGetErrorString(e),
+                                      (a->launch_err + b->launch_err).c_str());
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(OF_ERR_CUDA, "launch failed: %s; first failing launch: %s", cudaGetErrorString(e), (a->launch_err + b->launch_err).c_str());
+    a->last_launches = b->last_launches = n + 1;
+    CU_TRY(cudaEventRecord(a->last_done, st));
+    CU_TRY(cudaEventRecord(b->last_done, st));
+    a->last_stream = b->last_stream = st;
+    a->have_last = b->have_last = true;
+    return OF_OK;
 }
 
 int copy_plane_dense(const float *src, int pitch, int W, int H, float *dst, cudaStream_t st)
@@ -832,7 +888,8 @@ of_handle of_create(int width, int height, int levels, int window_radius, int it
     if (rc == OF_OK) {
         cudaError_t e = of_setup_attrs_hoisted(window_radius, SMEM_MAX);
         if (e == cudaSuccess) e = of_setup_attrs_masked(window_radius, SMEM_MAX);
-        if (e != cudaSuccess) rc = fail(OF_ERR_CUDA, "cudaFuncSetAttribute (hoisted / masked kernels): %s", cudaGetErrorString(e));
+        if (e == cudaSuccess) e = of_setup_attrs_dual(window_radius, SMEM_MAX);
+        if (e != cudaSuccess) rc = fail(OF_ERR_CUDA, "cudaFuncSetAttribute (hoisted / masked / two-pair kernels): %s", cudaGetErrorString(e));
     }
     if (rc == OF_OK) {
         c->sms = prop.multiProcessorCount;
@@ -894,6 +951,23 @@ int of_compute_u8(of_handle h, const uint8_t *I1, const uint8_t *I2, float *u, f
 int of_compute_u16(of_handle h, const uint16_t *I1, const uint16_t *I2, float *u, float *v, void *stream)
 {
     return compute_any(h, OF_DTYPE_U16, I1, I2, u, v, stream);
+}
+
+int of_compute_dual(of_handle ha, of_handle hb, int dtype, const void *I1a, const void *I2a, float *ua, float *va,
+                    const void *I1b, const void *I2b, float *ub, float *vb, void *stream)
+{
+    Job ja, jb;
+    int rc = make_pair_job(ha, dtype, I1a, I2a, ua, va, ja);
+    if (rc == OF_OK) rc = make_pair_job(hb, dtype, I1b, I2b, ub, vb, jb);
+    if (rc != OF_OK) return rc;
+    if (ha == hb) return fail(OF_ERR_INVALID_ARG, "of_compute_dual needs two different handles (each pair uses its handle's scratch)");
+    if (ha->device != hb->device) return fail(OF_ERR_INVALID_ARG, "the two handles belong to different devices");
+    if (!dual_eligible(ha, hb)) {                              // different problems, a mask, of_set_hoist, per-kernel mode: two ordinary solves
+        rc = submit_job(ha, ja, (cudaStream_t)stream);
+        if (rc == OF_OK) rc = submit_job(hb, jb, (cudaStream_t)stream);
+        return rc;
+    }
+    return submit_dual(ha, ja, hb, jb, (cudaStream_t)stream);
 }
 
 int of_set_conditioning(of_handle h, float eps_rel, float max_step_px)
@@ -1067,6 +1141,30 @@ int of_run_solve(of_handle h, int repeat, void *stream)
         cudaError_t e = cudaSuccess;
         DISPATCH_RB(h->R, h->ww.box, (e = launch_solve<R, BX>(h, nullptr, 0, 1, h->bench_out, h->bench_out + (size_t)h->W * h->H, st)));
         if (e != cudaSuccess) return fail(OF_ERR_CUDA, "solve launch failed: %s", cudaGetErrorString(e));
+    }
+    return OF_OK;
+}
+
+int of_run_solve_dual(of_handle ha, of_handle hb, int repeat, void *stream)
+{
+    if (!ha || !hb || repeat < 1) return fail(OF_ERR_INVALID_ARG, "bad argument");
+    if (!dual_eligible(ha, hb)) return fail(OF_ERR_STATE, "the two handles cannot share a launch (different problems, a mask, of_set_hoist or per-kernel mode)");
+    CU_TRY(cudaSetDevice(ha->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    of_context *hs[2] = {ha, hb};
+    SolveArgs sa[2];
+    for (int q = 0; q < 2; ++q) {
+        of_context *h = hs[q];
+        if (!h->bench_out) {                              // the discarded result gets a dense u, v pair of its own (first call only)
+            int rc = dev_alloc(h, (void **)&h->bench_out, sizeof(float) * 2 * (size_t)h->W * h->H);
+            if (rc != OF_OK) return rc;
+        }
+        fill_solve_args(h, 0, 1, h->bench_out, h->bench_out + (size_t)h->W * h->H, nullptr, sa[q]);
+    }
+    sa[1].prof = nullptr;
+    for (int i = 0; i < repeat; ++i) {
+        cudaError_t e = of_launch_solve_dual(ha->R, sa[0], sa[1], ha->sms, st);
+        if (e != cudaSuccess) return fail(OF_ERR_CUDA, "solve (two pairs) launch failed: %s", cudaGetErrorString(e));
     }
     return OF_OK;
 }

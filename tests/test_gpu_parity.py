@@ -769,3 +769,80 @@ def test_repeated_solves_are_bitwise_stable(torch, B, W, H, L, R, it, wt, hoist,
             else:
                 assert torch.equal(u, first[k][0]) and torch.equal(v, first[k][1]) and torch.equal(m, first[k][2])
         assert not torch.equal(first[0][0], first[1][0])
+
+
+# ---------------------------------------------------------------------------- throughput mode: two pairs in one launch (of_compute_dual)
+@pytest.mark.parametrize("W,H,L,R,it,wt,dt", [(320, 256, 3, 12, 4, GAUSS, "u8"), (256, 256, 1, 8, 4, BOX, "f32"), (130, 70, 2, 4, 3, BOX, "u8"),
+                                              (203, 131, 2, 5, 5, GAUSS, "u8"), (1280, 1024, 3, 12, 10, GAUSS, "u8"), (1280, 1024, 3, 8, 10, BOX, "u8"),
+                                              (1024, 1024, 2, 7, 6, BOX, "u16")])
+def test_dual_launch_matches_single_solves_bitwise(torch, B, W, H, L, R, it, wt, dt):
+    """of_compute_dual runs the passes of two different pairs alternately in one persistent kernel with split grid barriers
+    (csrc/of_solve_dual.cuh).  Each pair must come out exactly as of_compute gives it (fields and validity masks), also on the
+    second and third launch (barrier counters and ring parities carry over), and a single solve on the same handles afterwards
+    must still be right (the counters are returned to zero)."""
+    ca, cb = syn.config3(W, H, seed_offset=0), syn.config3(W, H, seed_offset=1)
+
+    def dev(a):
+        if dt == "f32":
+            return torch.from_numpy(a.astype(np.float32)).cuda()
+        if dt == "u16":
+            return torch.from_numpy((a.astype(np.uint16) * 16).view(np.int16)).cuda()
+        return torch.from_numpy(a).cuda()
+    d = [(dev(c.I1), dev(c.I2)) for c in (ca, cb)]
+    with B.OpticalFlow(W, H, L, R, it, wt) as ofa, B.OpticalFlow(W, H, L, R, it, wt) as ofb:
+        ref = []
+        for of, (i1, i2) in ((ofa, d[0]), (ofb, d[1])):
+            u, v = of.compute(i1, i2)
+            ref.append((u.clone(), v.clone(), of.validity().clone()))
+        torch.cuda.synchronize()
+        assert not torch.equal(ref[0][0], ref[1][0])
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            for rep in range(3):
+                ua, va, ub, vb = B.compute_dual(ofa, ofb, d[0][0], d[0][1], d[1][0], d[1][1])
+                ma, mb = ofa.validity(), ofb.validity()
+        s.synchronize()
+        assert ofa.last_launch_count() == 2 * (1 if L == 1 else L - 1) + 1
+        assert torch.equal(ua, ref[0][0]) and torch.equal(va, ref[0][1]) and torch.equal(ma, ref[0][2])
+        assert torch.equal(ub, ref[1][0]) and torch.equal(vb, ref[1][1]) and torch.equal(mb, ref[1][2])
+        # pairs swapped between the handles, then a single solve on each handle
+        with torch.cuda.stream(s):
+            ub2, vb2, ua2, va2 = B.compute_dual(ofa, ofb, d[1][0], d[1][1], d[0][0], d[0][1])
+            u1, v1 = ofb.compute(d[0][0], d[0][1])
+        s.synchronize()
+        assert torch.equal(ua2, ref[0][0]) and torch.equal(vb2, ref[1][1]) and torch.equal(u1, ref[0][0]) and torch.equal(v1, ref[0][1])
+
+
+def test_dual_launch_against_oracle(torch, B, oracle):
+    """The two fields of one of_compute_dual launch against the fp64 oracle, element by element (D23)."""
+    W, H, L, R, it, wt = 448, 320, 3, 7, 5, BOX
+    cs = [syn.config3(W, H, seed_offset=k) for k in (3, 4)]
+    with B.OpticalFlow(W, H, L, R, it, wt) as ofa, B.OpticalFlow(W, H, L, R, it, wt) as ofb:
+        ua, va, ub, vb = B.compute_dual(ofa, ofb, *[torch.from_numpy(x).cuda() for x in (cs[0].I1, cs[0].I2, cs[1].I1, cs[1].I2)])
+        ma, mb = ofa.validity(), ofb.validity()
+        torch.cuda.synchronize()
+    for c, u, v, m in ((cs[0], ua, va, ma), (cs[1], ub, vb, mb)):
+        ref = oracle.solve(c.I1, c.I2, L, R, it, wt)
+        assert_parity(u.cpu().numpy(), v.cpu().numpy(), m.cpu().numpy(), ref, "dual")
+
+
+def test_dual_launch_falls_back_and_rejects(torch, B):
+    """Handles that cannot share a launch (a mask on one of them) are solved one after the other with the same results; the same
+    handle twice is rejected."""
+    W, H, L, R, it, wt = 320, 256, 2, 6, 3, BOX
+    ca, cb = syn.config3(W, H, seed_offset=0), syn.config3(W, H, seed_offset=1)
+    d = [torch.from_numpy(x).cuda() for x in (ca.I1, ca.I2, cb.I1, cb.I2)]
+    mask = np.ones((H, W), np.uint8)
+    mask[40:90, 100:200] = 0
+    with B.OpticalFlow(W, H, L, R, it, wt) as ofa, B.OpticalFlow(W, H, L, R, it, wt) as ofb:
+        ofb.set_mask(mask)
+        ra = [t.clone() for t in ofa.compute(d[0], d[1])]
+        rb = [t.clone() for t in ofb.compute(d[2], d[3])]
+        ua, va, ub, vb = B.compute_dual(ofa, ofb, *d)
+        torch.cuda.synchronize()
+        assert torch.equal(ua, ra[0]) and torch.equal(va, ra[1]) and torch.equal(ub, rb[0]) and torch.equal(vb, rb[1])
+        assert float(ub[60, 150]) == 0.0 and ofa.last_launch_count() == 2            # an ordinary solve: pyramid + solve kernel
+        with pytest.raises(B.OptflowError):
+            B.compute_dual(ofa, ofa, *d)
+        with pytest.raises(B.OptflowError):
+            B.run_solve_dual(ofa, ofb)

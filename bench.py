@@ -252,6 +252,8 @@ def run_ours(args):
         if args.mask == "half":
             m[:, W // 2:] = 0
         of.set_mask(m)
+    if args.equalise > 0:                                       # eq. 2 pre-filter fused with the frame conversion (row f1)
+        of.set_equalisation(args.equalise)
     stream = torch.cuda.Stream(device=dev)
 
     def barrier():
@@ -297,7 +299,7 @@ def run_ours(args):
     # ---------------- throughput mode: two pairs per launch (of_compute_dual: the passes of two independent pairs alternate in one
     # persistent kernel and the grid barrier of one pair is waited for behind a pass of the other; results bit-identical to of_compute)
     dual = None
-    if not args.no_dual and nring >= 2 and args.mask == "none":      # (a masked handle cannot share a launch: of_compute_dual would fall back)
+    if not args.no_dual and nring >= 2 and args.mask == "none" and args.equalise == 0:      # (a masked handle cannot share a launch: of_compute_dual would fall back)
         of2 = B.OpticalFlow(*c0.create_args)
         npair2 = nring // 2
 
@@ -543,7 +545,7 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl, "levels": c0.levels, "window_radius": c0.window_radius, "iterations": c0.iterations,
                        "window": "gaussian" if c0.window_type == B.OF_WINDOW_GAUSSIAN else "box", "parallelism": "replicas only x%d" % world,
-                       "launch": launch_mode, "mask": args.mask,
+                       "launch": launch_mode, "mask": args.mask, "equalisation_radius": args.equalise,
                        "l2": "inputs and outputs rotate over a ring of %d pairs (%.0f MB; L2 is 126 MB); the %.0f MB of internal planes of the "
                              "finest level %s" % (nring, nring * (2 * px * esize + 8 * px) / 1e6, planes_mb,
                                                   "exceed L2: this workload is HBM bound" if planes_mb > 126 else "are L2 resident at this size")},
@@ -580,6 +582,7 @@ def main():
     ap.add_argument("--no-dual", action="store_true", help="skip the two-pairs-per-launch leg (of_compute_dual); the headline is then the single-pair launch")
     ap.add_argument("--mask", default="none", choices=["none", "step", "half"],
                     help="obstacle mask set on the handle (of_set_mask): step = synthetic.mask_backward_step (14 %% obstacle), half = right half of the frame")
+    ap.add_argument("--equalise", type=int, default=0, help="radius of the eq. 2 local-equalisation pre-filter (of_set_equalisation); 0 = off; the paper uses 5")
     ap.add_argument("--ring", type=int, default=RING, help="distinct input pairs / output buffers cycled through")
     args = ap.parse_args()
     if args.impl == "reference":

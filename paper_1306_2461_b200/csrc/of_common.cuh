@@ -5,7 +5,7 @@
 
 #define OFK_MAX_R 16
 
-// Profiling switches of the kernels (phases switched off one by one, profiles/r1_launch_overhead.md) exist in -DOF_PROFILE builds
+// Profiling switches of the kernels (phases switched off one by one, profiles/r2_notes.md, section 2) exist in -DOF_PROFILE builds
 // only: in the shipped build OF_DBG() is a compile-time 0 and the switches cost neither instructions nor registers.
 #ifdef OF_PROFILE
 #define OF_DBG(flags, bit) ((flags) & (bit))

@@ -231,7 +231,7 @@ __device__ __forceinline__ void k2_phase(const K2Params &p, unsigned char *smem_
         // then the arithmetic (other warps of the SM cover the two memory latencies)
         if (ntasks > 32 * K2_AHEAD_MIN_ROUNDS && ntasks <= 32 * K2_AHEAD_MAX_ROUNDS) {
         // wide tiles (three or more product rounds): the field values of ALL rounds of the tile are requested first, so that a
-        // round's gathers wait for one L2 round trip (I1 / I2) instead of two (u, v, then I2).  Measured (profiles/r1_experiments.md):
+        // round's gathers wait for one L2 round trip (I1 / I2) instead of two (u, v, then I2).  Measured (profiles/r2_notes.md, section 3):
         // level-0 K2 pass 16.0 -> 15.1 us at 1280x1024, 57.2 -> 50.1 us at 2048x2048; one-round tiles of the coarse levels lose
         // 0.4 us with it (unrolled guards), so they keep the rolled loop below.
         constexpr int MAXR = K2_AHEAD_MAX_ROUNDS;          // (wider tiles take the rolled loop below.  Every unrolled round is ~350 instructions

@@ -192,7 +192,7 @@ __device__ __forceinline__ void k3_phase(const CUtensorMap *tmS, const K3Params 
 
     if (warp == NWC) {
         // ===================== producer: the 32 lanes share the chunks of every run (lane k issues chunks k, k + 32, ...).
-        // One lane needs ~105 cycles per bulk tensor copy (expect_tx + issue; measured, profiles/r2_tma_issue.md), so a single
+        // One lane needs ~105 cycles per bulk tensor copy (expect_tx + issue; measured, profiles/r2_notes.md, section 4), so a single
         // lane delivered the ~40 chunks of a level-0 pass only after ~6700 cycles; 32 lanes have them in flight after ~2300.
         // Consumers wait on the full barrier of each chunk, so the order of issue does not matter.
         if (!OF_DBG(p.dbg, 1)) {

@@ -3,7 +3,7 @@
 //
 // Why: at 1280x1024 an iteration kernel runs 10-15 us and at the coarse levels 1-3 us, while a
 // kernel boundary costs 2-4 us on B200 (measured: an empty K2/K3 launch, back to back in a stream,
-// takes 4.1 us; profiles/r1_launch_overhead.md).  With ~65 launches per pair the boundaries were half
+// takes 4.1 us; profiles/r2_notes.md, section 2).  With ~65 launches per pair the boundaries were half
 // of the time.  Here one CTA per SM stays resident and the K2 pass (of_k2.cuh), the K3 pass
 // (of_k3.cuh) and the flow hand-down alternate, separated by a grid-wide barrier (one L2 atomic +
 // one acquire spin, < 1 us).  The decomposition of the method is unchanged: K2 still writes the five
@@ -36,7 +36,7 @@
 #define SOLVE_WARPS 12                       // 11 K3 consumers + 1 producer; all 12 work in the K2 pass
 #endif
 #ifndef SOLVE_CTAS_PER_SM
-#define SOLVE_CTAS_PER_SM 1                  // 2 in the half-SM build (optflow_half.cu): two solves of different pairs share every SM
+#define SOLVE_CTAS_PER_SM 1
 #endif
 
 struct LevelDesc {

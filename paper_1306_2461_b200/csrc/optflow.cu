@@ -182,7 +182,7 @@ template <int R> K2Plan plan_k2(int W, int H, int sms, double active = 1.0)   //
             const int nf_par = std::max(1, std::min(5, 32 / (nseg * nrp)));
             const int hs = (5 + nf_par - 1) / nf_par;                      // serial field sums per lane
             // Serial latency of a CTA's pass, in SM cycles, fitted to the in-kernel timeline (profiles/
-            // r1_experiments.md): a tile costs 1850 + 1300 per product round + (550 + 400 x warps sharing a
+            // r2_notes.md, section 3): a tile costs 1850 + 1300 per product round + (550 + 400 x warps sharing a
             // sub-partition's FMA pipe) per serial field sum; a CTA runs its tiles in waves of SOLVE_WARPS.
             const int tiles_cta = ((int)std::ceil(ntiles * active) + sms - 1) / sms;
             double cost = 0.0;

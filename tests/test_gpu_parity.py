@@ -846,3 +846,31 @@ def test_dual_launch_falls_back_and_rejects(torch, B):
             B.compute_dual(ofa, ofa, *d)
         with pytest.raises(B.OptflowError):
             B.run_solve_dual(ofa, ofb)
+
+
+@pytest.mark.parametrize("W,H,L,R,it,wt", [(320, 256, 3, 12, 4, GAUSS), (640, 512, 2, 8, 5, BOX), (1280, 1024, 3, 12, 10, GAUSS)])
+def test_dual_repeated_launches_are_bitwise_stable(torch, B, W, H, L, R, it, wt):
+    """Race evidence for the split grid barrier of of_solve_dual (compute-sanitizer is closed on this pool): 40 two-pair launches in a
+    row on the same two handles, the pairs swapping handles every launch and a single solve thrown in every eighth launch; every
+    field must reproduce the first one of its pair bit for bit."""
+    cs = [syn.config3(W, H, seed_offset=k) for k in (0, 1)]
+    d = [(torch.from_numpy(c.I1).cuda(), torch.from_numpy(c.I2).cuda()) for c in cs]
+    with B.OpticalFlow(W, H, L, R, it, wt) as ofa, B.OpticalFlow(W, H, L, R, it, wt) as ofb:
+        outs = []
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            for k in range(40):
+                p, q = (0, 1) if k % 2 == 0 else (1, 0)
+                ua, va, ub, vb = B.compute_dual(ofa, ofb, d[p][0], d[p][1], d[q][0], d[q][1])
+                outs += [(p, ua, va), (q, ub, vb)]
+                if k % 8 == 7:
+                    u1, v1 = ofa.compute(d[1][0], d[1][1])
+                    outs.append((1, u1, v1))
+        s.synchronize()
+        first = [None, None]
+        for p, u, v in outs:
+            if first[p] is None:
+                first[p] = (u, v)
+            else:
+                assert torch.equal(u, first[p][0]) and torch.equal(v, first[p][1])
+        assert not torch.equal(first[0][0], first[1][0])

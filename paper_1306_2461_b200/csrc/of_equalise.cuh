@@ -23,7 +23,7 @@ __host__ __device__ inline size_t eq_smem_bytes(int r, size_t elem)
 {
     const size_t pw = EQ_TW + 2 * r, ph = EQ_TH + 2 * r;
     const size_t s1 = elem == 4 ? 8 : 4, s2 = elem == 1 ? 4 : 8;           // sizeof(EqAcc<T>::S1), sizeof(EqAcc<T>::S2)
-    return (ph * pw * elem + 15) / 16 * 16 + ph * EQ_HS * (s1 + s2) + 16;  // patch + row sums
+    return (ph * (pw + 8) * elem + 15) / 16 * 16 + ph * EQ_HS * (s1 + s2) + 16;  // patch (rows of up to pw + 8 values: word-aligned staging) + row sums
 }
 
 // RT = the radius as a compile-time constant (the paper's 5: every loop unrolls) or 0 = run-time radius r_arg.
@@ -44,13 +44,29 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
     S1 *h1 = reinterpret_cast<S1 *>(h2 + (size_t)ph * EQ_HS + (sizeof(S2) == 4 ? (ph & 1) : 0));   // [ph][EQ_HS] row sums of I (8-byte aligned)
     T *patch = reinterpret_cast<T *>(h1 + (size_t)ph * EQ_HS);        // [ph][pw] raw values, 0 outside the image
     const int x0 = blockIdx.x * EQ_TW, y0 = blockIdx.y * EQ_TH;
-    for (int py = threadIdx.x >> 5; py < ph; py += 8) {               // a warp per patch row: coalesced, no divisions
-        const int gy = y0 - r + py;
-        const bool row_ok = gy >= 0 && gy < H;
-        const T *srow = src + (size_t)gy * W;
-        for (int px = threadIdx.x & 31; px < pw; px += 32) {
-            const int gx = x0 - r + px;
-            patch[py * pw + px] = (row_ok && gx >= 0 && gx < W) ? __ldg(srow + gx) : T(0);
+    // 8-bit frames whose rows are whole words are staged a word at a time: patch row = 80 bytes = columns x0-8 .. x0+71 (20 aligned
+    // 4-byte loads instead of 74 byte loads), value (gx, gy) at patch[py * pws + pofs + (gx - x0 + r)]
+    const bool vec = sizeof(T) == 1 && r <= 8 && (W & 3) == 0 && (reinterpret_cast<uintptr_t>(src) & 3) == 0;
+    const int pws = vec ? EQ_TW + 16 : pw, pofs = vec ? 8 - r : 0;
+    if (vec) {
+        constexpr int NWORD = (EQ_TW + 16) / 4;
+        unsigned *pw32 = reinterpret_cast<unsigned *>(patch);
+        for (int i = threadIdx.x; i < ph * NWORD; i += 256) {
+            const int py = i / NWORD, wx = i - py * NWORD;
+            const int gy = y0 - r + py, gx = x0 - 8 + 4 * wx;
+            unsigned word = 0u;
+            if (gy >= 0 && gy < H && gx >= 0 && gx < W) word = __ldg(reinterpret_cast<const unsigned *>(src + (size_t)gy * W + gx));
+            pw32[i] = word;
+        }
+    } else {
+        for (int py = threadIdx.x >> 5; py < ph; py += 8) {           // a warp per patch row: coalesced, no divisions
+            const int gy = y0 - r + py;
+            const bool row_ok = gy >= 0 && gy < H;
+            const T *srow = src + (size_t)gy * W;
+            for (int px = threadIdx.x & 31; px < pw; px += 32) {
+                const int gx = x0 - r + px;
+                patch[py * pw + px] = (row_ok && gx >= 0 && gx < W) ? __ldg(srow + gx) : T(0);
+            }
         }
     }
     __syncthreads();
@@ -58,7 +74,7 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
     // (add the entering value, subtract the leaving one: exact in integers); float frames re-sum every box.
     for (int i = threadIdx.x; i < ph * (EQ_TW / 8); i += 256) {
         const int py = i / (EQ_TW / 8), x8 = (i - py * (EQ_TW / 8)) * 8;
-        const T *p = patch + py * pw + x8;
+        const T *p = patch + py * pws + pofs + x8;
         S1 s = 0;
         S2 s2 = 0;
 #pragma unroll
@@ -112,9 +128,13 @@ __global__ void __launch_bounds__(256) k0_equalise(const T *__restrict__ srcA, c
             }
             if (gx >= W || gy >= H) continue;
             const int n = (min(gx + r, W - 1) - max(gx - r, 0) + 1) * (min(gy + r, H - 1) - max(gy - r, 0) + 1);
-            const T c = patch[(y + r) * pw + x + r];
+            const T c = patch[(y + r) * pws + pofs + x + r];
             float out;
-            if (sizeof(T) == 4) {                                          // float frames: fp64 moments
+            if (sizeof(T) == 1 && r <= 5) {                                // 8-bit frames, box of at most 11 x 11: every term fits 32 bits
+                const unsigned ns2 = (unsigned)n * (unsigned)s2, ss = (unsigned)s * (unsigned)s;   // <= 121 * 121 * 255^2 < 2^30
+                const int top = (int)c * n - (int)s;
+                out = ns2 > ss ? (float)top * rsqrtf((float)(ns2 - ss)) : 0.f;   // the same integers, hence the same floats, as the 64-bit form
+            } else if (sizeof(T) == 4) {                                          // float frames: fp64 moments
                 const double num = (double)n * (double)s2 - (double)s * (double)s;
                 out = num > 0.0 ? (float)(((double)c * n - (double)s) / sqrt(num)) : 0.f;
             } else {                                                       // integer frames: exact numerators

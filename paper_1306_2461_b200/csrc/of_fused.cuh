@@ -42,10 +42,11 @@ struct FusedParams {
     WinWeights ww;
     SolveParams sp;
     int zero_uv;
+    const uint8_t *mask;                   // obstacle mask of the level (pitch `pitch`; MK instantiation only): zero weight in the windows, no vector (M2, M3)
 };
 
 // Vertical window sums + solve + update of one tile out of the horizontally summed rows `hs` ([field][PH rows][tw]).
-template <int R, int SEG, bool BX>
+template <int R, int SEG, bool BX, bool MK>
 __device__ __forceinline__ void fused_vsolve(const FusedParams &p, const K3Params &p3, const float *hs, int x0, int y0, int tid, int nthr)
 {
     typedef FusedGeom<R> G;
@@ -63,6 +64,7 @@ __device__ __forceinline__ void fused_vsolve(const FusedParams &p, const K3Param
         for (int j = 0; j < SEG; ++j) {
             const int jj = min(j, nrows - 1) * p.pitch;
             mk[j] = 0x0101u;
+            if (MK) mk[j] = __ldg(reinterpret_cast<const unsigned short *>(p.mask + (size_t)gy0 * p.pitch + gx + jj));
             uu[j] = !p.zero_uv ? __ldcg(reinterpret_cast<const float2 *>(ui + jj)) : make_float2(0.f, 0.f);
             vv[j] = !p.zero_uv ? __ldcg(reinterpret_cast<const float2 *>(vi + jj)) : make_float2(0.f, 0.f);
         }
@@ -86,14 +88,15 @@ __device__ __forceinline__ void fused_vsolve(const FusedParams &p, const K3Param
             for (int f = 0; f < 5; ++f) win_vfinish<SEG, BOX>(acc[f], core[f]);
         };
         sum_rows(std::integral_constant<bool, BX>());
-        k3_solve_store<false, SEG>(p3, acc, uu, vv, mk, gx, gy0, nrows);
+        k3_solve_store<MK, SEG>(p3, acc, uu, vv, mk, gx, gy0, nrows);
     }
 }
 
 // One iteration of a level by the CTAs of the grid: CTA `cta` runs tiles cta, cta + ncta, ...  All threads of the CTA take part;
 // `smem` is the CTA's dynamic shared memory (at least FusedGeom<R>::smem_bytes(tw, th) bytes).
 // (__forceinline__ on purpose: as a __noinline__ function it spills and costs 4 us per iteration.)
-template <int R, bool BX>
+// MK = an obstacle mask is set (p.mask): masked products and outputs exactly as in the MK instantiations of K2 / K3; every tile is run.
+template <int R, bool BX, bool MK = false>
 __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned char *smem, int cta, int ncta)
 {
     typedef FusedGeom<R> G;
@@ -103,7 +106,7 @@ __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned c
     char *const prod = reinterpret_cast<char *>(smem);
     float *const hs = reinterpret_cast<float *>(smem + G::prod_bytes(tw, th));
     K2Params p2 = {};
-    p2.I1 = p.I1; p2.I2 = p.I2; p2.u = p.u_in; p2.v = p.v_in; p2.W = W; p2.H = H; p2.pitch = p.pitch; p2.zero_uv = p.zero_uv;
+    p2.I1 = p.I1; p2.I2 = p.I2; p2.u = p.u_in; p2.v = p.v_in; p2.W = W; p2.H = H; p2.pitch = p.pitch; p2.zero_uv = p.zero_uv; p2.mask = p.mask;
     K3Params p3 = {};
     p3.u_in = p.u_in; p3.v_in = p.v_in; p3.u_out = p.u_out; p3.v_out = p.v_out; p3.valid = p.valid; p3.det = p.det;
     p3.W = W; p3.H = H; p3.pitch = p.pitch; p3.out_pitch = p.out_pitch; p3.sp = p.sp; p3.zero_uv = p.zero_uv;
@@ -139,14 +142,14 @@ __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned c
             if (x >= 0 && x < W && y >= 0 && y < H) {
                 K2In in;
                 if (have_uv) {
-                    in = k2_load<false, false>(p2, x, y);
+                    in = k2_load<MK, false>(p2, x, y);
                     in.u0 = u0; in.u1 = u1; in.v0 = v0; in.v1 = v1;
                 } else {
-                    in = k2_load<false>(p2, x, y);
+                    in = k2_load<MK>(p2, x, y);
                 }
                 K2Tap tp[4];
                 k2_task_gather(p2, in, x, y, tp);
-                k2_task_products<false>(p2, in, x, y, tp, o);
+                k2_task_products<MK>(p2, in, x, y, tp, o);
             } else {
 #pragma unroll
                 for (int f = 0; f < 5; ++f) o[f] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -184,7 +187,7 @@ __device__ __forceinline__ void fused_iteration(const FusedParams &p, unsigned c
         __syncthreads();
         // ---------------- vertical window sums + solve + update: lane task = 2 columns x K3_SEG rows (shorter tasks on small tiles, so
         // that every thread has one, were measured slower: 14.2 against 12.5 us per iteration at 640x512)
-        fused_vsolve<R, K3_SEG, BX>(p, p3, hs, x0, y0, tid, nthr);
+        fused_vsolve<R, K3_SEG, BX, MK>(p, p3, hs, x0, y0, tid, nthr);
         __syncthreads();                                   // the buffers are reused by the CTA's next tile
     }
 }

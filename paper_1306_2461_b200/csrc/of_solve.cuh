@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, SOLVE_CTAS_PER_SM) of_solve_
         MaskDesc M = {};
         if (MK) M = a.md[l];
         // fused coarse level (of_fused.cuh): the field alternates between (u, v) and (u2, v2); start so that the last iteration ends in (u, v)
-        const bool fused = !MK && L.f_ntiles > 0;
+        const bool fused = L.f_ntiles > 0;
         LevelDesc Lw = L;
         if (fused && (a.iterations & 1)) { Lw.u = L.u2; Lw.v = L.v2; }
         if (l < top) {
@@ -260,8 +260,8 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, SOLVE_CTAS_PER_SM) of_solve_
                 const bool last = (l == 0 && it == a.iterations - 1);
                 const FusedParams fp = {L.pyr[a.s1], L.pyr[a.s2], ui, vi, last ? a.u_out : uo, last ? a.v_out : vo, last ? a.valid : nullptr,
                                         last ? a.det : nullptr, L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.f_tw, L.f_th, L.f_tiles_x, L.f_ntiles,
-                                        a.ww, a.sp, (l == top && it == 0) ? 1 : 0};
-                fused_iteration<R, BX>(fp, solve_smem, cta, ncta);
+                                        a.ww, a.sp, (l == top && it == 0) ? 1 : 0, M.mask};
+                fused_iteration<R, BX, MK>(fp, solve_smem, cta, ncta);
                 prof_stamp(a, pi);                               // (four stamps per iteration, as in the two-pass form)
                 prof_stamp(a, pi);
                 prof_stamp(a, pi);

@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(32 * SOLVE_WARPS, 1) of_solve_dual(const __gri
                     float *ui = from_uv ? L.u : L.u2, *vi = from_uv ? L.v : L.v2, *uo = from_uv ? L.u2 : L.u, *vo = from_uv ? L.v2 : L.v;
                     const FusedParams fp = {L.pyr[a.s1], L.pyr[a.s2], ui, vi, last ? a.u_out : uo, last ? a.v_out : vo, last ? a.valid : nullptr,
                                             last ? a.det : nullptr, L.W, L.H, L.pitch, last ? a.out_pitch : L.pitch, L.f_tw, L.f_th, L.f_tiles_x, L.f_ntiles,
-                                            a0.ww, a0.sp, (l == top && it == 0) ? 1 : 0};
+                                            a0.ww, a0.sp, (l == top && it == 0) ? 1 : 0, nullptr};
                     fused_iteration<R, BX>(fp, solve_smem, cta, ncta);
                     dual_end_pass(a.gbar, o.gbar, DUAL_OTHER_TARGET(q, last), nullptr);
                 }

@@ -688,7 +688,7 @@ int upload_level_descs(of_context *c)
         hl[l] = {{c->pyr[0][l], c->pyr[1][l]}, c->u[l], c->v[l], c->lv[l].W, c->lv[l].H, c->lv[l].pitch,
                  c->k2[l].nseg, c->k2[l].nrp, c->k2[l].tiles_y, c->k2[l].ntiles, c->k3[l].nrb, c->k3[l].ntasks,
                  c->k2s_nuy[l], c->k2s_nunits[l], k2s_magic(c->k2s_nuy[l]), c->u2[l], c->v2[l],
-                 c->f_tw[l], c->f_th[l], c->f_tiles_x[l], (c->fuse_coarse && !c->md[l].mask) ? c->f_ntiles[l] : 0};
+                 c->f_tw[l], c->f_th[l], c->f_tiles_x[l], c->fuse_coarse ? c->f_ntiles[l] : 0};
     CU_TRY(cudaMemcpy(c->d_lv, hl, sizeof(LevelDesc) * c->levels, cudaMemcpyHostToDevice));
     CU_TRY(cudaMemcpy(c->d_md, c->md, sizeof(MaskDesc) * c->levels, cudaMemcpyHostToDevice));
     return OF_OK;

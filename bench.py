@@ -492,7 +492,12 @@ def run_ours(args):
                     "note": "algorithmic bytes over time against the HBM copy peak, as SURVEY.md 8(d) defines the bar; at 1280x1024 the planes are "
                             "L2 resident (see traffic: the single-pair capture x pairs per launch), so the limiter is latency / issue rate, not DRAM: "
                             "against the measured L2-resident streaming rate of the same byte mix the fraction is frac_of_l2_streaming",
-                    "frac_of_l2_streaming": ach / L2_STREAM_GBPS, "l2_streaming_GBps": L2_STREAM_GBPS}
+                    "frac_of_l2_streaming": ach / L2_STREAM_GBPS, "l2_streaming_GBps": L2_STREAM_GBPS,
+                    # the second bound of DESIGN.md sec. 7: fp32 FMA of the two window sums, 2 x 5 x (2R+1) per pixel-iteration, against
+                    # 128 FMA per clock per SM (measured 127, profiles/r2_notes.md sec. 1) at the sampled SM clock
+                    "window_fma_per_launch": 10.0 * (2 * c0.window_radius + 1) * pix_iters * npairs,
+                    "window_fma_frac_of_fma_peak": 10.0 * (2 * c0.window_radius + 1) * pix_iters * npairs / (solve_us_ * 1e-6) / (torch.cuda.get_device_properties(dev).multi_processor_count * 128 * mhz * 1e6),
+                    "window_fma_note": "direct (2R+1)-tap sums; box windows of radius >= 4 take the add-only form with about half as many operations"}
             it0 = {"bytes": 72 * px * npairs, "us": iter_us, "GB/s": iter_gbs, "frac_of_peak": iter_gbs / peak,
                    "phases_us": {"k2_pass": float(med[0]), "barrier_1": float(med[1]), "k3_pass": float(med[2]), "barrier_2": float(med[3])},
                    "how": "in-kernel SM cycle stamps (of_solve_timeline, max over CTAs) / sampled SM clock; median over iterations" +

@@ -119,6 +119,58 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def trace_overlap(run):
+    """Device activity of one pipeline pass as CUPTI sees it (torch.profiler; nsys is not in this image): how much of the host<->device
+    copy time runs under a kernel of the library, i.e. the overlap of Fig. 4."""
+    from torch.profiler import ProfilerActivity, profile
+    from torch.autograd import DeviceType
+    with profile(activities=[ProfilerActivity.CUDA]) as prof:
+        run()
+    kern, h2d, d2h = [], [], []
+    for e in prof.events():
+        if e.device_type != DeviceType.CUDA:
+            continue
+        iv = (float(e.time_range.start), float(e.time_range.end))
+        n = e.name.lower()
+        if "memcpy htod" in n:
+            h2d.append(iv)
+        elif "memcpy dtoh" in n:
+            d2h.append(iv)
+        elif "memcpy" not in n and "memset" not in n:
+            kern.append(iv)
+
+    def union(iv):
+        out = []
+        for a, b in sorted(iv):
+            if out and a <= out[-1][1]:
+                out[-1][1] = max(out[-1][1], b)
+            else:
+                out.append([a, b])
+        return out
+
+    def length(iv):
+        return sum(b - a for a, b in iv)
+
+    def inter(x, y):
+        i = j = 0
+        tot = 0.0
+        while i < len(x) and j < len(y):
+            a, b = max(x[i][0], y[j][0]), min(x[i][1], y[j][1])
+            if b > a:
+                tot += b - a
+            if x[i][1] < y[j][1]:
+                i += 1
+            else:
+                j += 1
+        return tot
+    ku, hu, du = union(kern), union(h2d), union(d2h)
+    span = max(b for _, b in ku + hu + du) - min(a for a, _ in ku + hu + du) if (ku or hu or du) else 0.0
+    return {"tool": "torch.profiler (CUPTI activity records of every stream of the process)", "span_us": span,
+            "kernels": len(kern), "kernel_busy_us": length(ku), "kernel_busy_frac_of_span": length(ku) / span if span else None,
+            "h2d_copies": len(h2d), "h2d_us": length(hu), "h2d_under_kernels_frac": inter(hu, ku) / length(hu) if hu else None,
+            "d2h_copies": len(d2h), "d2h_us": length(du), "d2h_under_kernels_frac": inter(du, ku) / length(du) if du else None}
+
+
 def shard_pairs(n_pairs, rank, world):
     """Round-robin frame pairs over ranks (independent fields -> replicas)."""
     return list(range(rank, n_pairs, world))
@@ -374,6 +426,7 @@ def run_ours(args):
     # ---------------- end to end through the public pipeline API: host buffers in, host fields out
     checksum = 0.0
     e2e = None
+    overlap_trace = None
     if not args.no_e2e:
         if streaming:
             # config 5 as BASELINE.json:11 states it: the frames sit in ordinary (pageable) host memory, every frame is uploaded once
@@ -404,6 +457,8 @@ def run_ours(args):
             barrier()
             dt, got = run_stream()
             e2e_ms, e2e_steps = dt * 1e3, got
+            if args.trace_overlap and rank == 0:
+                overlap_trace = trace_overlap(run_stream)                 # one more pass, under the profiler (not timed)
             api = "of_stream_open(CONSECUTIVE, host results) / acquire+fill / submit / result; 256 frames from pageable host memory, wall clock first submit -> last result"
             h2d, d2h = W * H * esize, 8 * W * H + W * H
         else:
@@ -439,7 +494,7 @@ def run_ours(args):
             h2d, d2h = 2 * W * H * esize, 8 * W * H + W * H
         e2e_ms = reduce_max_time(e2e_ms, dist, dev)
         e2e = {"value": world * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "steps": e2e_steps, "api": api, "checksum": checksum,
+               "steps": e2e_steps, "api": api, "checksum": checksum, "overlap_trace": overlap_trace,
                "overlap": "serial sum per pair would be solve %.0f us + H2D %.0f us + D2H %.0f us at ~25 GB/s pinned PCIe; measured %.0f us per pair" %
                           (ms / args.steps * 1e3, h2d / 25e3, d2h / 25e3, e2e_ms / e2e_steps * 1e3)}
 
@@ -594,6 +649,8 @@ def main():
     ap.add_argument("--mask", default="none", choices=["none", "step", "half"],
                     help="obstacle mask set on the handle (of_set_mask): step = synthetic.mask_backward_step (14 %% obstacle), half = right half of the frame")
     ap.add_argument("--equalise", type=int, default=0, help="radius of the eq. 2 local-equalisation pre-filter (of_set_equalisation); 0 = off; the paper uses 5")
+    ap.add_argument("--trace-overlap", action="store_true",
+                    help="config5 only: one extra pipeline pass under torch.profiler; reports how much of the copy time runs under kernels")
     ap.add_argument("--ring", type=int, default=RING, help="distinct input pairs / output buffers cycled through")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -442,7 +442,7 @@ def run_ours(args):
                     slot = of.stream_acquire()
                     np.copyto(slot, f)
                     of.stream_submit()
-                    if k >= 2:                                            # stay one field behind: upload k+1 overlaps solve k
+                    if k >= 3:                                            # stay two fields behind: uploads k+1, k+2 overlap solve k
                         _, u, v = of.stream_result()
                         checksum += float(u[H // 2, W // 2]) + float(v[H // 2, W // 2])
                         got += 1
@@ -462,7 +462,7 @@ def run_ours(args):
             api = "of_stream_open(CONSECUTIVE, host results) / acquire+fill / submit / result; 256 frames from pageable host memory, wall clock first submit -> last result"
             h2d, d2h = W * H * esize, 8 * W * H + W * H
         else:
-            e2e_steps = max(args.steps // 2, 200)
+            e2e_steps = min(5000, max(args.steps // 2, 200, int(50.0 / (ms / args.steps))))   # at least 200 pairs and about 50 ms of device work
 
             def pump(n):
                 nonlocal checksum
@@ -473,7 +473,7 @@ def run_ours(args):
                     np.copyto(slot[1], pairs[i % nring][1])
                     of.stream_submit()
                     pending += 1
-                    if pending == 2:
+                    if pending == 3:
                         _, u, v = of.stream_result()
                         checksum += float(u[H // 2, W // 2]) + float(v[H // 2, W // 2])
                         pending -= 1

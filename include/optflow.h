@@ -238,7 +238,7 @@ int of_upsample_flow(const float *uc, const float *vc, int wc, int hc, float *u,
                      int height, void *stream);
 
 /* ---------------------------------------------------------------------------------------------
- * Frame pipeline (Fig. 4 schemes; "(5)" in BASELINE.json:5): pinned host slots,
+ * Frame pipeline (Fig. 4 schemes; "(5)" in BASELINE.json:5): four pinned host slots,
  * cudaMemcpyAsync on a side stream, events; uploading frame k+1 overlaps solving pair k, and the
  * download of field k overlaps solving pair k+1.
  *   OF_STREAM_CONSECUTIVE: each submitted frame is converted and pyramided once and used as I2 of
@@ -252,8 +252,9 @@ int of_stream_open(of_handle h, int dtype, int mode, int result_on_host);
 /* Pinned host buffer for the next submit (W*H elements, x2 in PAIRS mode); the caller fills it.
  * Blocks until that slot's previous upload has completed.  NULL on error. */
 void *of_stream_acquire(of_handle h);
-/* Enqueue upload (+ solve + download) of the slot last acquired.  Returns OF_ERR_STATE if more than
- * two produced fields have not been collected with of_stream_result. */
+/* Enqueue upload (+ solve + download) of the slot last acquired.  Up to three produced fields may be waiting to be collected
+ * (small frames need that depth to keep the GPU busy: a field's way through upload, solve and download takes longer than two
+ * solves); returns OF_ERR_STATE if three already are. */
 int of_stream_submit(of_handle h);
 /* Wait for the oldest uncollected field.  *u, *v point to H x W fp32 (host or device per
  * of_stream_open), valid until the second-next of_stream_result call.  *pair_index (optional)

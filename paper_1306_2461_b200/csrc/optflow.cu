@@ -65,16 +65,16 @@ struct Job {
 struct GraphEntry { Job job; cudaGraphExec_t exec; unsigned long long stamp; int launches; };
 
 constexpr int N_PYR = 2;       // pyramid slots
-constexpr int N_PIN = 2;       // pinned upload slots ("double buffering")
-constexpr int N_RES = 4;       // result ring
+constexpr int N_PIN = 4;       // pinned upload slots (the paper's double buffering, two deeper: up to N_RES - 2 = 3 fields may be in flight)
+constexpr int N_RES = 5;       // result ring: a returned field stays valid until the second-next of_stream_result call
 
 struct Pipeline {
     bool open = false;
     int dtype = 0, mode = 0, host_result = 0;
     size_t frame_bytes = 0, slot_bytes = 0, field_bytes = 0;
     cudaStream_t s_copy = nullptr, s_comp = nullptr, s_down = nullptr;
-    void *pin[N_PIN] = {nullptr, nullptr};
-    void *raw[N_PIN] = {nullptr, nullptr};
+    void *pin[N_PIN] = {};
+    void *raw[N_PIN] = {};
     float *res_dev[N_RES] = {};            // per slot: u, v (2 x field_bytes), then the validity bytes (W*H)
     float *res_host[N_RES] = {};
     cudaEvent_t h2d_done[N_PIN] = {}, cvt_done[N_PIN] = {}, solve_done[N_RES] = {}, d2h_done[N_RES] = {};
@@ -1307,8 +1307,8 @@ int of_stream_submit(of_handle h)
     Pipeline &p = h->pipe;
     if (p.cur_slot < 0) return fail(OF_ERR_STATE, "of_stream_submit without of_stream_acquire");
     const bool yields = (p.mode == OF_STREAM_PAIRS) || p.submitted >= 1;
-    if (yields && p.produced - p.collected >= 2)
-        return fail(OF_ERR_STATE, "two fields are waiting: call of_stream_result before submitting more");
+    if (yields && p.produced - p.collected >= N_RES - 2)
+        return fail(OF_ERR_STATE, "%d fields are waiting: call of_stream_result before submitting more", N_RES - 2);
     CU_TRY(cudaSetDevice(h->device));
     const int s = p.cur_slot;
     // upload: the device slot must have been consumed by the conversion of the frame it held before

@@ -155,12 +155,23 @@ def test_stream_pairs_mode(torch, B, oracle):
             idx, u, v = of.stream_result()
             assert idx == rep
             assert_parity(u, v, None, ref, "pairs-mode")
-        # overflow protection: a third uncollected field is refused
-        for rep in range(2):
+        # three fields may be in flight (include/optflow.h); a fourth uncollected one is refused, and the three come out right and in order
+        for rep in range(3):
             slot = of.stream_acquire(); slot[0] = c.I1; slot[1] = c.I2; of.stream_submit()
         of.stream_acquire()
         with pytest.raises(B.OptflowError):
             of.stream_submit()
+        held = []
+        for rep in range(3):
+            idx, u, v = of.stream_result()
+            assert idx == 5 + rep
+            held.append((u, v))
+            assert_parity(u, v, None, ref, "pairs-mode, three in flight")
+        # a returned field stays valid until the second-next of_stream_result call: the last two are still intact
+        assert np.array_equal(held[1][0], held[2][0]) and np.array_equal(held[1][1], held[2][1])
+        of.stream_submit()                                   # the slot acquired above
+        idx, u, v = of.stream_result()
+        assert idx == 8
         of.stream_close()
 
 
